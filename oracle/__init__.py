@@ -1,0 +1,116 @@
+"""CPU oracle of the sort + trigger path -- TEST INFRASTRUCTURE, not product code.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+import this package.  It never imports paper_1411_3968_b200's CUDA binding and shares no code
+with it; the numpy record dtypes below are re-declared from the paper's description of the
+fixed-size hit structure and BASELINE.json configs[0].
+
+`build()` compiles oracle/tt_oracle.cpp with g++ into oracle/liboracle.so.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tt_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+HIT = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
+EVENT = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
+                  ("seed_begin", "<u4"), ("n_seeds", "<u4")])
+F_Q, F_LC, F_L1, F_L2STAR, F_L2, F_INEVT = 1, 2, 4, 8, 16, 32
+
+
+class _Params(ctypes.Structure):
+    _fields_ = [("lc_window_ps", ctypes.c_int64), ("l2_window_ps", ctypes.c_int64),
+                ("event_half_ps", ctypes.c_int64), ("l2_multiplicity", ctypes.c_uint32),
+                ("l2_mode", ctypes.c_uint32), ("q_thresh", ctypes.c_uint32), ("reserved", ctypes.c_uint32)]
+
+
+def build(force: bool = False) -> str:
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-o", _LIB, _SRC])
+    return _LIB
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = ctypes.CDLL(build())
+    return _lib
+
+
+def _p(a):
+    return a.ctypes.data_as(ctypes.c_void_p) if a is not None else None
+
+
+def _mk_params(q_thresh, lc_window_ps, l2_window_ps, l2_multiplicity, l2_mode, event_half_ps):
+    return _Params(int(lc_window_ps), int(l2_window_ps), int(event_half_ps), int(l2_multiplicity),
+                   int(l2_mode), int(q_thresh), 0)
+
+
+def sort(hits: np.ndarray, seg_offsets: np.ndarray):
+    """-> (sorted hits, perm)"""
+    hits = np.ascontiguousarray(hits, dtype=HIT)
+    seg = np.ascontiguousarray(seg_offsets, dtype=np.uint32)
+    n = hits.shape[0]
+    out = np.empty_like(hits)
+    perm = np.empty(n, dtype=np.uint32)
+    rc = lib().oracle_sort(_p(hits), _p(out), _p(perm), ctypes.c_uint32(n), _p(seg), ctypes.c_uint32(len(seg) - 1))
+    assert rc == 0
+    return out, perm
+
+
+@dataclass
+class TriggerResult:
+    flags: np.ndarray
+    seeds: np.ndarray
+    status: int
+
+
+def trigger(sorted_hits: np.ndarray, seg_offsets: np.ndarray, n_pmt: int, n_tower: int, ppt: int,
+            pair_block: np.ndarray, blocks: np.ndarray, *, q_thresh=300, lc_window_ps=20_000,
+            l2_window_ps=3_000_000, l2_multiplicity=5, l2_mode=0, event_half_ps=3_000_000) -> TriggerResult:
+    h = np.ascontiguousarray(sorted_hits, dtype=HIT)
+    seg = np.ascontiguousarray(seg_offsets, dtype=np.uint32)
+    pb = np.ascontiguousarray(pair_block, dtype=np.int32)
+    bl = np.ascontiguousarray(blocks, dtype=np.int32)
+    n = h.shape[0]
+    flags = np.zeros(n, dtype=np.uint8)
+    seeds = np.zeros(max(n, 1), dtype=np.uint32)
+    ns = ctypes.c_uint32(0)
+    st = ctypes.c_int32(0)
+    prm = _mk_params(q_thresh, lc_window_ps, l2_window_ps, l2_multiplicity, l2_mode, event_half_ps)
+    rc = lib().oracle_trigger(_p(h), ctypes.c_uint32(n), _p(seg), ctypes.c_uint32(len(seg) - 1),
+                              ctypes.c_uint32(n_pmt), ctypes.c_uint32(n_tower), ctypes.c_uint32(ppt),
+                              _p(pb), _p(bl), ctypes.byref(prm), _p(flags), _p(seeds), ctypes.byref(ns),
+                              ctypes.byref(st))
+    if rc != 0:
+        raise ValueError("oracle_trigger: invalid parameters")
+    return TriggerResult(flags, seeds[: ns.value].copy(), st.value)
+
+
+def events(sorted_hits: np.ndarray, seg_offsets: np.ndarray, seeds: np.ndarray, *, event_half_ps=3_000_000,
+           flags: np.ndarray | None = None):
+    """-> events array (EVENT dtype); ORs F_INEVT into flags in place when given."""
+    h = np.ascontiguousarray(sorted_hits, dtype=HIT)
+    seg = np.ascontiguousarray(seg_offsets, dtype=np.uint32)
+    sd = np.ascontiguousarray(seeds, dtype=np.uint32)
+    ev = np.zeros(max(len(sd), 1), dtype=EVENT)
+    ne = ctypes.c_uint32(0)
+    prm = _mk_params(0, 0, 0, 1, 0, event_half_ps)
+    if flags is not None:
+        assert flags.dtype == np.uint8 and flags.flags.c_contiguous
+    rc = lib().oracle_events(_p(h), ctypes.c_uint32(h.shape[0]), _p(seg), ctypes.c_uint32(len(seg) - 1), _p(sd),
+                             ctypes.c_uint32(len(sd)), ctypes.byref(prm), _p(ev), ctypes.byref(ne), _p(flags))
+    if rc != 0:
+        raise ValueError("oracle_events: invalid parameters")
+    return ev[: ne.value].copy()

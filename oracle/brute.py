@@ -1,0 +1,101 @@
+"""Brute-force checkers that pin oracle/tt_oracle.cpp -- TEST INFRASTRUCTURE.
+
+Written separately from the oracle (different language, different formulation: exhaustive
+pair / subset enumeration straight from the definitions in BASELINE.json:north_star) so that
+a mistake cannot be shared.  Tiny inputs only (O(n^2) and O(C(n,N))).
+"""
+from __future__ import annotations
+
+import itertools
+
+import numpy as np
+
+
+def seg_id(n: int, seg_offsets) -> np.ndarray:
+    s = np.zeros(n, dtype=np.int64)
+    for k in range(len(seg_offsets) - 1):
+        s[int(seg_offsets[k]):int(seg_offsets[k + 1])] = k
+    return s
+
+
+def l1_flags(h: np.ndarray, seg_offsets, q_thresh: int, lc_ps: int) -> np.ndarray:
+    """north_star: 'a charge-over-threshold test and a same-floor local coincidence (L1)'.
+    All ordered pairs, no use of the time order."""
+    n = len(h)
+    sg = seg_id(n, seg_offsets)
+    t = h["t_ps"].astype(object)  # python ints: no overflow
+    out = np.zeros(n, dtype=np.uint8)
+    for i in range(n):
+        f = 1 if int(h["charge"][i]) >= q_thresh else 0
+        for j in range(n):
+            if j == i or sg[j] != sg[i]:
+                continue
+            if h["floor"][j] == h["floor"][i] and h["pmt_id"][j] != h["pmt_id"][i] and abs(t[j] - t[i]) <= lc_ps:
+                f |= 2
+                break
+        if f:
+            f |= 4
+        out[i] = f
+    return out
+
+
+def l2_flags(h: np.ndarray, seg_offsets, l1: np.ndarray, table: np.ndarray, W: int, N: int):
+    """north_star: 'at least N L1 hits pairwise satisfying |dt| <= dt_max(pmt_i, pmt_j)' within
+    the <= 3 us window.  Returns (star, clique) boolean arrays by enumerating every pair and every
+    N-subset of L1 hits.  table is the dense (P,P) integer table, -1 = never."""
+    n = len(h)
+    sg = seg_id(n, seg_offsets)
+    idx = [i for i in range(n) if l1[i]]
+    t = [int(x) for x in h["t_ps"]]
+    pm = [int(x) for x in h["pmt_id"]]
+    P = table.shape[0]
+
+    def edge(a, b):
+        if sg[a] != sg[b] or pm[a] >= P or pm[b] >= P:
+            return False
+        lim = int(table[pm[a], pm[b]])
+        if lim < 0:
+            return False
+        return abs(t[a] - t[b]) <= min(lim, W)
+
+    star = np.zeros(n, dtype=bool)
+    clique = np.zeros(n, dtype=bool)
+    for a in idx:
+        deg = sum(1 for b in idx if b != a and edge(a, b))
+        star[a] = deg >= N - 1
+    if N == 1:
+        clique[idx] = True
+        return star, clique
+    for sub in itertools.combinations(idx, N):
+        if all(edge(a, b) for a, b in itertools.combinations(sub, 2)):
+            clique[list(sub)] = True
+    return star, clique
+
+
+def event_groups(seed_t, seed_seg, H: int):
+    """Union of the closed windows [t-H, t+H] of the seeds, per segment: two seeds share an event
+    iff they are linked by a chain of overlapping (or touching) windows.  Union-find over all pairs.
+    Returns a list of (segment, t_start, t_end, [seed positions])."""
+    m = len(seed_t)
+    parent = list(range(m))
+
+    def find(x):
+        while parent[x] != x:
+            parent[x] = parent[parent[x]]
+            x = parent[x]
+        return x
+
+    for a in range(m):
+        for b in range(a + 1, m):
+            # windows [ta-H, ta+H] and [tb-H, tb+H] intersect iff |ta-tb| <= 2H
+            if seed_seg[a] == seed_seg[b] and abs(int(seed_t[a]) - int(seed_t[b])) <= 2 * H:
+                parent[find(a)] = find(b)
+    groups: dict[int, list[int]] = {}
+    for a in range(m):
+        groups.setdefault(find(a), []).append(a)
+    out = []
+    for members in groups.values():
+        ts = [int(seed_t[a]) for a in members]
+        out.append((int(seed_seg[members[0]]), min(ts) - H, max(ts) + H, sorted(members)))
+    out.sort(key=lambda e: (e[0], e[1]))
+    return out

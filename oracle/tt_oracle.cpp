@@ -1,0 +1,210 @@
+// oracle/tt_oracle.cpp -- TEST INFRASTRUCTURE, not product code.
+//
+// Plain, slow, single-threaded CPU definition of the hot path of the online muon trigger of
+// "Parallel Neutrino Triggers using GPUs for an Underwater Telescope" (arxiv 1411.3968),
+// as scoped by BASELINE.json:north_star.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may load this library.  It shares no code, headers,
+// tables or helpers with paper_1411_3968_b200/csrc (the CUDA path); the record layouts below
+// are re-declared here on purpose.
+//
+// What each function follows:
+//   oracle_sort     PAPER.md:51-53 (sect. 4.2 "First we sort the hits in time"); north_star "put
+//                   them in global timestamp order (a merge of the per-PMT time-ordered streams)".
+//                   The plain definition: std::stable_sort by t_ps inside each segment
+//                   (reading R2: ties keep input order).
+//   oracle_trigger  PAPER.md:27-29 (sect. 3: charge over threshold; time-space correlation within
+//                   3 us), PAPER.md:61-64 (SC/FC coincidences, QTRIG) with the windows and the
+//                   pairwise L2 condition of north_star / BASELINE.json configs[0].
+//   oracle_events   PAPER.md:23 ("a 6 us time window ... centered at the time of the trigger
+//                   seed"), PAPER.md:67 ("all hits within +-3 us are tagged").
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force pair / subset enumeration written
+// separately in oracle/brute.py, numpy stable argsort, Poisson closed forms, N-in-TW special
+// case, interval-union brute force, hand-written boundary cases.  No function
+// here is "parity unpinned".
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+struct Hit {
+    int64_t t_ps;
+    uint16_t pmt_id, floor, charge, pad;
+};
+static_assert(sizeof(Hit) == 16, "hit record is 16 bytes");
+
+struct Params {
+    int64_t lc_window_ps;
+    int64_t l2_window_ps;
+    int64_t event_half_ps;
+    uint32_t l2_multiplicity;
+    uint32_t l2_mode;  // 0 clique, 1 star
+    uint32_t q_thresh;
+    uint32_t reserved;
+};
+static_assert(sizeof(Params) == 40, "params layout");
+
+struct Event {
+    int64_t t_start, t_end;
+    uint32_t hit_begin, hit_end, seed_begin, n_seeds;
+};
+static_assert(sizeof(Event) == 32, "event record is 32 bytes");
+
+enum : uint8_t { F_Q = 1, F_LC = 2, F_L1 = 4, F_L2STAR = 8, F_L2 = 16, F_INEVT = 32 };
+enum : int32_t { S_BAD_PMT = 8 };
+
+struct Geo {
+    uint32_t n_pmt, n_tower, ppt;
+    const int32_t* pair_block;  // [n_tower*n_tower], -1 = unconnected
+    const int32_t* blocks;      // [n_blocks][ppt][ppt] ps
+};
+
+// dtmax(pmt_a, pmt_b): the integer causality table; -1 = never an edge.
+int64_t dtmax(const Geo& g, uint32_t a, uint32_t b) {
+    if (a >= g.n_pmt || b >= g.n_pmt) return -1;
+    const uint32_t ta = a / g.ppt, tb = b / g.ppt;
+    const int32_t blk = g.pair_block[(size_t)ta * g.n_tower + tb];
+    if (blk < 0) return -1;
+    return g.blocks[((size_t)blk * g.ppt + (a % g.ppt)) * g.ppt + (b % g.ppt)];
+}
+
+// Is there a subset of `need` members of cand[from..], pairwise adjacent?  Plain recursion.
+bool has_clique(const std::vector<std::vector<uint8_t>>& adj, const std::vector<int>& cand, int need) {
+    if (need == 0) return true;
+    if ((int)cand.size() < need) return false;
+    for (size_t k = 0; k < cand.size(); ++k) {
+        const int v = cand[k];
+        std::vector<int> rest;
+        for (size_t m = k + 1; m < cand.size(); ++m)
+            if (adj[v][cand[m]]) rest.push_back(cand[m]);
+        if (has_clique(adj, rest, need - 1)) return true;
+    }
+    return false;
+}
+
+}  // namespace
+
+extern "C" {
+
+// Stable ascending sort by t_ps inside each segment.  perm[k] = input index of out[k].
+int oracle_sort(const Hit* in, Hit* out, uint32_t* perm, uint32_t n, const uint32_t* seg_off, uint32_t n_seg) {
+    std::vector<uint32_t> idx(n);
+    for (uint32_t i = 0; i < n; ++i) idx[i] = i;
+    for (uint32_t s = 0; s < n_seg; ++s)
+        std::stable_sort(idx.begin() + seg_off[s], idx.begin() + seg_off[s + 1],
+                         [in](uint32_t a, uint32_t b) { return in[a].t_ps < in[b].t_ps; });
+    for (uint32_t k = 0; k < n; ++k) {
+        out[k] = in[idx[k]];
+        if (perm) perm[k] = idx[k];
+    }
+    return 0;
+}
+
+// L1 (Q | LC), L2 (clique / star) and the ascending seed list on time-sorted hits.
+// seeds must have room for n entries.  Returns 0, or -1 for invalid parameters.
+int oracle_trigger(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n_seg, uint32_t n_pmt,
+                   uint32_t n_tower, uint32_t ppt, const int32_t* pair_block, const int32_t* blocks,
+                   const Params* p, uint8_t* flags, uint32_t* seeds, uint32_t* n_seeds, int32_t* status) {
+    if (p->l2_multiplicity < 1 || p->lc_window_ps < 0 || p->l2_window_ps < 0) return -1;
+    const Geo g{n_pmt, n_tower, ppt, pair_block, blocks};
+    const int64_t LC = p->lc_window_ps, W = p->l2_window_ps;
+    const int N = (int)p->l2_multiplicity;
+    *status = 0;
+    std::memset(flags, 0, n);
+    uint32_t ns = 0;
+    for (uint32_t s = 0; s < n_seg; ++s) {
+        const int64_t a = seg_off[s], b = seg_off[s + 1];
+        // ---- L1: charge over threshold, or a same-floor hit on another PMT within LC ----
+        for (int64_t i = a; i < b; ++i) {
+            uint8_t f = 0;
+            if (h[i].charge >= p->q_thresh) f |= F_Q;
+            bool lc = false;
+            for (int64_t j = i - 1; j >= a && h[i].t_ps - h[j].t_ps <= LC; --j)
+                if (h[j].floor == h[i].floor && h[j].pmt_id != h[i].pmt_id) lc = true;
+            for (int64_t j = i + 1; j < b && h[j].t_ps - h[i].t_ps <= LC; ++j)
+                if (h[j].floor == h[i].floor && h[j].pmt_id != h[i].pmt_id) lc = true;
+            if (lc) f |= F_LC;
+            if (f) f |= F_L1;
+            flags[i] = f;
+        }
+        // ---- L2 on the L1 hits of this segment ----
+        std::vector<int64_t> l1;
+        for (int64_t i = a; i < b; ++i)
+            if (flags[i] & F_L1) {
+                l1.push_back(i);
+                if (h[i].pmt_id >= n_pmt) *status |= S_BAD_PMT;
+            }
+        const int64_t m = (int64_t)l1.size();
+        auto edge = [&](int64_t x, int64_t y) {  // x, y index l1[]
+            const Hit &hx = h[l1[x]], &hy = h[l1[y]];
+            const int64_t d = hx.t_ps > hy.t_ps ? hx.t_ps - hy.t_ps : hy.t_ps - hx.t_ps;
+            const int64_t lim = std::min<int64_t>(dtmax(g, hx.pmt_id, hy.pmt_id), W);
+            return lim >= 0 && d <= lim;
+        };
+        for (int64_t x = 0; x < m; ++x) {
+            std::vector<int64_t> nb;  // neighbours of x, ascending
+            int64_t lo = x;
+            while (lo > 0 && h[l1[x]].t_ps - h[l1[lo - 1]].t_ps <= W) --lo;
+            for (int64_t y = lo; y < m && h[l1[y]].t_ps - h[l1[x]].t_ps <= W; ++y)
+                if (y != x && edge(x, y)) nb.push_back(y);
+            const int k = (int)nb.size();
+            if (k < N - 1) continue;
+            flags[l1[x]] |= F_L2STAR;
+            bool l2 = true;
+            if (p->l2_mode == 0) {
+                std::vector<std::vector<uint8_t>> adj(k, std::vector<uint8_t>(k, 0));
+                for (int u = 0; u < k; ++u)
+                    for (int v = 0; v < k; ++v)
+                        if (u != v) adj[u][v] = edge(nb[u], nb[v]);
+                std::vector<int> cand(k);
+                for (int u = 0; u < k; ++u) cand[u] = u;
+                l2 = has_clique(adj, cand, N - 1);
+            }
+            if (l2) flags[l1[x]] |= F_L2;
+        }
+        // ---- seeds: ascending sorted-array indices of L2 hits ----
+        for (int64_t i = a; i < b; ++i)
+            if (flags[i] & F_L2) seeds[ns++] = (uint32_t)i;
+    }
+    *n_seeds = ns;
+    return 0;
+}
+
+// Merge the [t-H, t+H] windows of consecutive seeds (closed intervals; merge iff gap <= 2H),
+// never across a segment.  events must have room for n_seeds entries.
+int oracle_events(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n_seg, const uint32_t* seeds,
+                  uint32_t n_seeds, const Params* p, Event* events, uint32_t* n_events, uint8_t* flags) {
+    (void)n;
+    const int64_t H = p->event_half_ps;
+    if (H < 0) return -1;
+    uint32_t ne = 0, k = 0;
+    for (uint32_t s = 0; s < n_seg; ++s) {
+        const uint32_t a = seg_off[s], b = seg_off[s + 1];
+        while (k < n_seeds && seeds[k] < b) {
+            uint32_t first = k, last = k;
+            while (last + 1 < n_seeds && seeds[last + 1] < b &&
+                   h[seeds[last + 1]].t_ps - h[seeds[last]].t_ps <= 2 * H)
+                ++last;
+            Event e;
+            e.t_start = h[seeds[first]].t_ps - H;
+            e.t_end = h[seeds[last]].t_ps + H;
+            uint32_t lo = seeds[first], hi = seeds[last] + 1;
+            while (lo > a && h[lo - 1].t_ps >= e.t_start) --lo;  // lower_bound(t >= t_start)
+            while (hi < b && h[hi].t_ps <= e.t_end) ++hi;        // upper_bound(t <= t_end)
+            e.hit_begin = lo;
+            e.hit_end = hi;
+            e.seed_begin = first;
+            e.n_seeds = last - first + 1;
+            if (flags)
+                for (uint32_t i = lo; i < hi; ++i) flags[i] |= F_INEVT;
+            events[ne++] = e;
+            k = last + 1;
+        }
+    }
+    *n_events = ne;
+    return 0;
+}
+
+}  // extern "C"
