@@ -1,0 +1,149 @@
+/* tt.h -- C ABI of the B200 tower-trigger library (libtt.so).
+ *
+ * The hot path of the online muon trigger of "Parallel Neutrino Triggers using GPUs for an
+ * Underwater Telescope" (arxiv 1411.3968; citations are lines of PAPER.md), as scoped by
+ * BASELINE.json:north_star:
+ *
+ *   tt_sort_slice      PAPER.md:51-53 (sect. 4.2 "First we sort the hits in time"; the per-PMT streams
+ *                      are already time-ordered)            -- stable time sort
+ *   tt_trigger_slice   PAPER.md:27-29 (sect. 3: charge over threshold, time-space correlation within
+ *                      3 us), PAPER.md:61-64 (coincidences, QTRIG)       -- L1, L2, seed list
+ *   tt_extract_events  PAPER.md:23 ("a 6 us time window ... centered at the time of the trigger seed"),
+ *                      PAPER.md:67 ("all hits within +-3 us are tagged") -- event-window merge, tagging
+ *
+ * Conventions
+ *   d_*   device pointers (caller-owned; the library never allocates in the three hot calls)
+ *   h_*   host pointers; `p`, `g`, `ws_bytes` are host pointers too
+ *   All hot calls are asynchronous: they enqueue kernels on `stream` (a cudaStream_t passed as
+ *   void*) and return.  The return value covers argument errors only (TT_OK / TT_E_*).
+ *   Data-dependent conditions are OR-ed into *d_status (device int32, zeroed by the caller or by
+ *   a previous call's owner), to be read after synchronising: TT_S_* bits.
+ *   Workspace: call with d_ws == NULL to get the required size in *ws_bytes (nothing is enqueued);
+ *   otherwise *ws_bytes must be >= that size.  d_ws must be 256-byte aligned.
+ *   Indices are uint32: n < 2^32 - 2^20.
+ *   Segments: d_seg_offsets[n_seg+1] (device) splits the hit array into independent slices
+ *   (no sort movement, coincidence or event crosses a segment).  h_seg_offsets is the same array
+ *   on the host (needed to size launches); both must agree.
+ */
+#ifndef TT_H_
+#define TT_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Fixed-size hit record ("a fixed size structure": charge, time, DU identification);
+ * 16 bytes, 16-byte aligned.  t_ps: picoseconds, any int64.  floor: global floor id (tower*floors+f).
+ * charge: 0.01 p.e. units.  pad: carried through unchanged. */
+typedef struct {
+    int64_t t_ps;
+    uint16_t pmt_id, floor, charge, pad;
+} tt_hit;
+
+/* Trigger parameters (BASELINE.json configs[0]); 40 bytes, no implicit padding. */
+typedef struct {
+    int64_t lc_window_ps;     /* L1 same-floor coincidence window, inclusive (20000)              */
+    int64_t l2_window_ps;     /* W: an L2 edge needs |dt| <= min(dtmax, W), inclusive (3000000)    */
+    int64_t event_half_ps;    /* H: event window is [t_seed - H, t_seed + H] (3000000)             */
+    uint32_t l2_multiplicity; /* N >= 1, counts the hit itself; N <= TT_MAX_MULTIPLICITY           */
+    uint32_t l2_mode;         /* 0 = clique ("N L1 hits pairwise causal"), 1 = star                */
+    uint32_t q_thresh;        /* Q bit <=> charge >= q_thresh (0.01 p.e.; PAPER.md:64 QTRIG)       */
+    uint32_t reserved;        /* must be 0                                                         */
+} tt_params;
+
+/* One merged event window; 32 bytes.  Times are unclipped; [hit_begin, hit_end) indexes the sorted
+ * hit array, [seed_begin, seed_begin + n_seeds) indexes the seed list. */
+typedef struct {
+    int64_t t_start, t_end;
+    uint32_t hit_begin, hit_end, seed_begin, n_seeds;
+} tt_event;
+
+/* per-hit flag byte */
+enum { TT_Q = 1, TT_LC = 2, TT_L1 = 4, TT_L2STAR = 8, TT_L2 = 16, TT_INEVT = 32 };
+/* return codes */
+enum { TT_OK = 0, TT_E_INVAL = -1, TT_E_CUDA = -2, TT_E_WORKSPACE = -3 };
+/* *d_status bits */
+enum {
+    TT_S_OK = 0,
+    TT_S_SEED_OVERFLOW = 1,  /* n_seeds > seed_cap: *d_n_seeds is the true count, first seed_cap valid */
+    TT_S_EVENT_OVERFLOW = 2, /* likewise for events                                                   */
+    TT_S_RUN_UNSORTED = 4,   /* a run given by d_run_offsets is not non-decreasing: output unspecified */
+    TT_S_BAD_PMT = 8,        /* an L1 hit has pmt_id >= n_pmt (it has no L2 edges)                     */
+    TT_S_DENSITY = 16        /* an L1 hit has more than TT_MAX_NEIGHBOURS causal neighbours: its L2STAR
+                                bit is exact, its clique-mode L2 bit is not decided (left clear)       */
+};
+#define TT_MAX_MULTIPLICITY 16
+#define TT_MAX_NEIGHBOURS 256
+
+/* Causality table dtmax[pmt_a][pmt_b] in integer ps (BASELINE.json configs[0]: d_ij*n/c + 20 ns,
+ * precomputed by the caller), block-sparse by tower pair:
+ *   dtmax(a, b) = h_blocks[h_pair_block[ta*n_tower + tb]][a % ppt][b % ppt],  ta = a / ppt,
+ * -1 (block id or entry) = the pair is never an edge.  One tower: n_tower = 1, h_pair_block = {0}.
+ * The table is copied to the device; tt_geometry_destroy frees it.  Returns TT_E_INVAL for a
+ * non-symmetric table, a block id out of range, or n_pmt != n_tower * pmts_per_tower. */
+typedef struct tt_geometry tt_geometry;
+int tt_geometry_create(tt_geometry** g, uint32_t n_pmt, uint32_t n_tower, uint32_t pmts_per_tower,
+                       const int32_t* h_pair_block, const int32_t* h_blocks, uint32_t n_blocks);
+int tt_geometry_destroy(tt_geometry* g);
+
+/* Stable ascending sort of d_in[n] by t_ps inside each segment (ties keep input order) into
+ * d_out[n] (a pure permutation of whole 16-byte records; d_out must not alias d_in).
+ * d_perm (nullable): d_perm[k] = input index of d_out[k].
+ * d_run_offsets[n_runs+1] (nullable, with its host copy h_run_offsets): consecutive, already
+ * non-decreasing runs covering [0, n) that never straddle a segment (the per-PMT streams).  Given,
+ * the library merges the runs; NULL, it radix-sorts arbitrary input.  A run that is not sorted sets
+ * TT_S_RUN_UNSORTED. */
+int tt_sort_slice(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n,
+                  const uint32_t* d_seg_offsets, const uint32_t* h_seg_offsets, uint32_t n_seg,
+                  const uint32_t* d_run_offsets, const uint32_t* h_run_offsets, uint32_t n_runs,
+                  void* d_ws, size_t* ws_bytes, int32_t* d_status, void* stream);
+
+/* L1 (Q | same-floor coincidence on another PMT within lc_window), L2 (clique or star over the
+ * causality table within l2_window) and the ascending seed list on time-sorted hits.
+ * d_flags[n] is overwritten (TT_Q..TT_L2 bits).  d_seeds[seed_cap] receives the sorted-array
+ * indices of the L2 hits, *d_n_seeds the true count. */
+int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets,
+                     const uint32_t* h_seg_offsets, uint32_t n_seg, const tt_geometry* g,
+                     const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds, uint32_t seed_cap,
+                     uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes, int32_t* d_status, void* stream);
+
+/* Merge the closed windows [t-H, t+H] of consecutive seeds (merge <=> gap <= 2H, never across a
+ * segment) into d_events[event_cap]; *d_n_events = true count.  The seed list is read from the
+ * device (d_seeds, *d_n_seeds as written by tt_trigger_slice; at most seed_cap entries are used).
+ * d_flags (nullable): TT_INEVT is OR-ed into the flags of every hit inside an event.
+ * d_gather (nullable, room for n records): the hits of all events, concatenated in order;
+ * *d_n_gathered (nullable) = their number. */
+int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets,
+                      const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* d_seeds,
+                      const uint32_t* d_n_seeds, uint32_t seed_cap, const tt_params* p,
+                      tt_event* d_events, uint32_t event_cap, uint32_t* d_n_events, uint8_t* d_flags,
+                      tt_hit* d_gather, uint32_t* d_n_gathered, void* d_ws, size_t* ws_bytes,
+                      int32_t* d_status, void* stream);
+
+/* Whole-slice convenience with HOST buffers (end-to-end use and timing; not a hot call).
+ * tt_host_ctx_create allocates, once, device buffers and workspaces for slices of up to max_n hits,
+ * max_seg segments and max_runs runs, and an internal stream; tt_host_ctx_destroy frees them.
+ * tt_process_host copies the hits and offsets to the device (h_in pinned or pageable), runs
+ * tt_sort_slice -> tt_trigger_slice -> tt_extract_events (with INEVT tagging), copies back the
+ * sorted hits (h_sorted nullable), the flags (h_flags nullable), the first min(n_seeds, seed_cap)
+ * seeds and min(n_events, event_cap) events, and synchronises.
+ * h_counts[3] = {n_seeds, n_events, status}.  h_run_offsets NULL = unsorted input. */
+typedef struct tt_host_ctx tt_host_ctx;
+int tt_host_ctx_create(tt_host_ctx** c, uint32_t max_n, uint32_t max_seg, uint32_t max_runs, uint32_t seed_cap,
+                       uint32_t event_cap);
+int tt_host_ctx_destroy(tt_host_ctx* c);
+int tt_process_host(tt_host_ctx* c, const tt_hit* h_in, tt_hit* h_sorted, uint8_t* h_flags, uint32_t n,
+                    const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* h_run_offsets,
+                    uint32_t n_runs, const tt_geometry* g, const tt_params* p, uint32_t* h_seeds,
+                    tt_event* h_events, uint32_t* h_counts);
+
+/* Library version / build string (static storage). */
+const char* tt_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TT_H_ */

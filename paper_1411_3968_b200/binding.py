@@ -1,0 +1,264 @@
+"""Thin ctypes binding of libtt.so (include/tt.h).  Argument marshalling only: every step of the
+path runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams.
+
+There is no CPU fallback: importing works without a GPU (so the ABI can be inspected), but every
+compute call needs the library and a CUDA device and raises otherwise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+import numpy as np
+import torch
+
+from . import _build
+
+c_u32, c_i32, c_vp, c_sz = ctypes.c_uint32, ctypes.c_int32, ctypes.c_void_p, ctypes.c_size_t
+
+TT_Q, TT_LC, TT_L1, TT_L2STAR, TT_L2, TT_INEVT = 1, 2, 4, 8, 16, 32
+TT_OK, TT_E_INVAL, TT_E_CUDA, TT_E_WORKSPACE = 0, -1, -2, -3
+TT_S_SEED_OVERFLOW, TT_S_EVENT_OVERFLOW, TT_S_RUN_UNSORTED, TT_S_BAD_PMT, TT_S_DENSITY = 1, 2, 4, 8, 16
+
+EXPORTS = ["tt_version", "tt_geometry_create", "tt_geometry_destroy", "tt_sort_slice", "tt_trigger_slice",
+           "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host"]
+
+HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
+EVENT_DTYPE = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
+                        ("seed_begin", "<u4"), ("n_seeds", "<u4")])
+
+
+class TTParams(ctypes.Structure):
+    """Mirror of tt_params (40 bytes)."""
+    _fields_ = [("lc_window_ps", ctypes.c_int64), ("l2_window_ps", ctypes.c_int64),
+                ("event_half_ps", ctypes.c_int64), ("l2_multiplicity", c_u32), ("l2_mode", c_u32),
+                ("q_thresh", c_u32), ("reserved", c_u32)]
+
+
+assert ctypes.sizeof(TTParams) == 40
+
+
+class TTError(RuntimeError):
+    pass
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load(build: bool = True):
+    """Load libtt.so (building it if stale).  Raises if it cannot be built or loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.build() if build else _build.LIB
+        if not os.path.exists(path):
+            raise TTError(f"{path} is missing: run __graft_entry__.build()")
+        L = ctypes.CDLL(path)
+        L.tt_version.restype = ctypes.c_char_p
+        for name in EXPORTS[1:]:
+            getattr(L, name).restype = ctypes.c_int
+        _lib = L
+    return _lib
+
+
+def _check(rc: int, what: str):
+    if rc != TT_OK:
+        raise TTError(f"{what} failed: {({-1: 'TT_E_INVAL', -2: 'TT_E_CUDA', -3: 'TT_E_WORKSPACE'}).get(rc, rc)}")
+
+
+def _need_cuda():
+    if not torch.cuda.is_available():
+        raise TTError("no CUDA device: the tower-trigger path has no CPU fallback")
+
+
+def _dp(t: torch.Tensor | None):
+    return c_vp(t.data_ptr()) if t is not None else c_vp(0)
+
+
+def _hp(a: np.ndarray | None):
+    return a.ctypes.data_as(c_vp) if a is not None else c_vp(0)
+
+
+def _stream() -> c_vp:
+    return c_vp(torch.cuda.current_stream().cuda_stream)
+
+
+def make_params(q_thresh=300, lc_window_ps=20_000, l2_window_ps=3_000_000, l2_multiplicity=5, l2_mode=0,
+                event_half_ps=3_000_000) -> TTParams:
+    return TTParams(int(lc_window_ps), int(l2_window_ps), int(event_half_ps), int(l2_multiplicity), int(l2_mode),
+                    int(q_thresh), 0)
+
+
+class Geometry:
+    """Owns a tt_geometry handle (device copy of the block-sparse causality table)."""
+
+    def __init__(self, n_pmt: int, n_tower: int, pmts_per_tower: int, pair_block: np.ndarray, blocks: np.ndarray):
+        _need_cuda()
+        L = load()
+        pb = np.ascontiguousarray(pair_block, dtype=np.int32)
+        bl = np.ascontiguousarray(blocks, dtype=np.int32)
+        self.n_pmt, self.n_tower, self.ppt = int(n_pmt), int(n_tower), int(pmts_per_tower)
+        self._h = c_vp(0)
+        torch.cuda.init()
+        torch.zeros(1, device="cuda")  # make sure the primary context exists
+        rc = L.tt_geometry_create(ctypes.byref(self._h), c_u32(n_pmt), c_u32(n_tower), c_u32(pmts_per_tower), _hp(pb),
+                                  _hp(bl), c_u32(bl.shape[0]))
+        _check(rc, "tt_geometry_create")
+
+    @property
+    def handle(self):
+        return self._h
+
+    def close(self):
+        if self._h:
+            load().tt_geometry_destroy(self._h)
+            self._h = c_vp(0)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def hits_to_device(hits: np.ndarray) -> torch.Tensor:
+    """(n,) HIT_DTYPE numpy -> (n, 2) int64 CUDA tensor (16-byte records)."""
+    _need_cuda()
+    h = np.ascontiguousarray(hits, dtype=HIT_DTYPE)
+    return torch.from_numpy(h.view(np.int64).reshape(-1, 2).copy()).cuda()
+
+
+def hits_to_host(t: torch.Tensor) -> np.ndarray:
+    return t.cpu().numpy().reshape(-1).view(HIT_DTYPE).copy()
+
+
+def _offsets(o) -> tuple[np.ndarray, torch.Tensor]:
+    h = np.ascontiguousarray(o, dtype=np.uint32)
+    d = torch.from_numpy(h.view(np.int32).copy()).cuda()
+    return h, d
+
+
+class Offsets:
+    """Host + device copies of an offsets array (uint32[k+1])."""
+
+    def __init__(self, o):
+        self.h, self.d = _offsets(o)
+        self.count = len(self.h) - 1
+
+
+def _ws(query, what) -> torch.Tensor:
+    need = c_sz(0)
+    _check(query(c_vp(0), ctypes.byref(need)), what + " (workspace query)")
+    return torch.empty(max(int(need.value), 256), dtype=torch.uint8, device="cuda")
+
+
+def tt_sort_slice(d_in: torch.Tensor, d_out: torch.Tensor, d_perm: torch.Tensor | None, seg: Offsets,
+                  runs: Offsets | None, d_status: torch.Tensor, ws: torch.Tensor | None = None) -> torch.Tensor:
+    """Enqueue tt_sort_slice on the current stream.  Returns the workspace tensor used (reusable)."""
+    _need_cuda()
+    L = load()
+    n = d_in.shape[0]
+
+    def call(wsp, nbytes):
+        return L.tt_sort_slice(_dp(d_in), _dp(d_out), _dp(d_perm), c_u32(n), _dp(seg.d), _hp(seg.h), c_u32(seg.count),
+                               _dp(runs.d) if runs else c_vp(0), _hp(runs.h) if runs else c_vp(0),
+                               c_u32(runs.count if runs else 0), wsp, nbytes, _dp(d_status), _stream())
+
+    if ws is None:
+        ws = _ws(call, "tt_sort_slice")
+    nb = c_sz(ws.numel())
+    _check(call(_dp(ws), ctypes.byref(nb)), "tt_sort_slice")
+    return ws
+
+
+def tt_trigger_slice(d_sorted: torch.Tensor, seg: Offsets, geo: Geometry, params: TTParams, d_flags: torch.Tensor,
+                     d_seeds: torch.Tensor, d_n_seeds: torch.Tensor, d_status: torch.Tensor,
+                     ws: torch.Tensor | None = None) -> torch.Tensor:
+    _need_cuda()
+    L = load()
+    n = d_sorted.shape[0]
+
+    def call(wsp, nbytes):
+        return L.tt_trigger_slice(_dp(d_sorted), c_u32(n), _dp(seg.d), _hp(seg.h), c_u32(seg.count), geo.handle,
+                                  ctypes.byref(params), _dp(d_flags), _dp(d_seeds), c_u32(d_seeds.numel()),
+                                  _dp(d_n_seeds), wsp, nbytes, _dp(d_status), _stream())
+
+    if ws is None:
+        ws = _ws(call, "tt_trigger_slice")
+    nb = c_sz(ws.numel())
+    _check(call(_dp(ws), ctypes.byref(nb)), "tt_trigger_slice")
+    return ws
+
+
+def tt_extract_events(d_sorted: torch.Tensor, seg: Offsets, d_seeds: torch.Tensor, d_n_seeds: torch.Tensor,
+                      params: TTParams, d_events: torch.Tensor, d_n_events: torch.Tensor,
+                      d_flags: torch.Tensor | None, d_gather: torch.Tensor | None, d_n_gathered: torch.Tensor | None,
+                      d_status: torch.Tensor, ws: torch.Tensor | None = None) -> torch.Tensor:
+    _need_cuda()
+    L = load()
+    n = d_sorted.shape[0]
+
+    def call(wsp, nbytes):
+        return L.tt_extract_events(_dp(d_sorted), c_u32(n), _dp(seg.d), _hp(seg.h), c_u32(seg.count), _dp(d_seeds),
+                                   _dp(d_n_seeds), c_u32(d_seeds.numel()), ctypes.byref(params), _dp(d_events),
+                                   c_u32(d_events.shape[0]), _dp(d_n_events), _dp(d_flags), _dp(d_gather),
+                                   _dp(d_n_gathered), wsp, nbytes, _dp(d_status), _stream())
+
+    if ws is None:
+        ws = _ws(call, "tt_extract_events")
+    nb = c_sz(ws.numel())
+    _check(call(_dp(ws), ctypes.byref(nb)), "tt_extract_events")
+    return ws
+
+
+@dataclass
+class SliceResult:
+    sorted: np.ndarray
+    perm: np.ndarray
+    flags: np.ndarray
+    seeds: np.ndarray
+    n_seeds: int
+    events: np.ndarray
+    n_events: int
+    status: int
+    gathered: np.ndarray | None = None
+
+
+def process_slice(hits: np.ndarray, seg_offsets, run_offsets, geo: Geometry, params: TTParams, seed_cap=None,
+                  event_cap=None, gather=False) -> SliceResult:
+    """Convenience for tests: upload, run the three calls, download everything."""
+    _need_cuda()
+    n = len(hits)
+    seg = Offsets(seg_offsets)
+    runs = Offsets(run_offsets) if run_offsets is not None else None
+    d_in = hits_to_device(hits)
+    d_out = torch.empty_like(d_in)
+    d_perm = torch.empty(max(n, 1), dtype=torch.int32, device="cuda")
+    d_status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    seed_cap = n if seed_cap is None else seed_cap
+    event_cap = n if event_cap is None else event_cap
+    d_flags = torch.zeros(max(n, 1), dtype=torch.uint8, device="cuda")
+    d_seeds = torch.zeros(max(seed_cap, 1), dtype=torch.int32, device="cuda")[:seed_cap]
+    d_ns = torch.zeros(1, dtype=torch.int32, device="cuda")
+    d_ev = torch.zeros((max(event_cap, 1), 4), dtype=torch.int64, device="cuda")[:event_cap]
+    d_ne = torch.zeros(1, dtype=torch.int32, device="cuda")
+    d_g = torch.zeros((max(n, 1), 2), dtype=torch.int64, device="cuda") if gather else None
+    d_ng = torch.zeros(1, dtype=torch.int32, device="cuda") if gather else None
+    tt_sort_slice(d_in, d_out, d_perm, seg, runs, d_status)
+    tt_trigger_slice(d_out, seg, geo, params, d_flags, d_seeds, d_ns, d_status)
+    tt_extract_events(d_out, seg, d_seeds, d_ns, params, d_ev, d_ne, d_flags, d_g, d_ng, d_status)
+    torch.cuda.synchronize()
+    ns, ne = int(d_ns.item()) & 0xFFFFFFFF, int(d_ne.item()) & 0xFFFFFFFF
+    res = SliceResult(
+        sorted=hits_to_host(d_out), perm=d_perm.cpu().numpy().view(np.uint32)[:n].copy(),
+        flags=d_flags.cpu().numpy()[:n].copy(), seeds=d_seeds.cpu().numpy().view(np.uint32)[: min(ns, seed_cap)].copy(),
+        n_seeds=ns, events=d_ev.cpu().numpy().reshape(-1).view(EVENT_DTYPE)[: min(ne, event_cap)].copy(), n_events=ne,
+        status=int(d_status.item()))
+    if gather:
+        ng = int(d_ng.item()) & 0xFFFFFFFF
+        res.gathered = hits_to_host(d_g)[:ng]
+    return res

@@ -1,0 +1,208 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, bit-exact (integer work).
+Element-by-element: sorted records, permutation, flags, seeds, events."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from cases import case_arrays, directed_cases
+from paper_1411_3968_b200 import workload as W
+from util import oracle_chain, single_tower_geo
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1411_3968_b200 import binding
+
+    binding.load()
+    return binding
+
+
+def _geo(B, g):
+    return B.Geometry(g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks)
+
+
+def _prm(B, p):
+    return B.make_params(p.q_thresh, p.lc_window_ps, p.l2_window_ps, p.l2_multiplicity, p.l2_mode, p.event_half_ps)
+
+
+def _compare(r, o):
+    assert r.sorted.tobytes() == o["sorted"].tobytes()
+    assert (r.perm == o["perm"]).all()
+    bad = np.nonzero(r.flags != o["flags"])[0]
+    assert len(bad) == 0, (bad[:10], r.flags[bad[:10]], o["flags"][bad[:10]])
+    assert r.n_seeds == len(o["seeds"]) and (r.seeds == o["seeds"]).all()
+    assert r.n_events == len(o["events"])
+    assert r.events.tobytes() == o["events"].tobytes()
+    assert (r.status & 8) == (o["status"] & 8)
+
+
+CASES = directed_cases()
+
+
+@pytest.mark.parametrize("c", CASES, ids=[c["name"] for c in CASES])
+def test_directed_cases(c, B, oracle_lib):
+    h, seg = case_arrays(c)
+    g = single_tower_geo(c["table"])
+    p = W.Params(**c["params"])
+    o = oracle_chain(h, seg, g, p)
+    geo = _geo(B, g)
+    for runs in (None, np.arange(len(h) + 1, dtype=np.uint32)):  # radix path; every hit its own run
+        r = B.process_slice(h, seg, runs, geo, _prm(B, p))
+        _compare(r, o)
+        e = c["expect"]
+        if "flags" in e:
+            assert r.flags.tolist() == e["flags"]
+        if "seeds" in e:
+            assert r.seeds.tolist() == e["seeds"]
+        if "events" in e:
+            assert [tuple(int(x) for x in ev) for ev in r.events] == e["events"]
+        assert r.status == 0
+
+
+@pytest.mark.parametrize("cfg,ts,ss", [(0, 0.25, 1), (1, 0.1, 1), (2, 0.004, 1), (3, 0.02, 8 / 64), (4, 0.002, 1)])
+@pytest.mark.parametrize("mode", [0, 1])
+def test_configs_scaled(cfg, ts, ss, mode, B, oracle_lib):
+    """The five BASELINE.json configs at oracle-speed sizes (several tiles, ragged tails)."""
+    w = W.make_config(cfg, time_scale=ts, seg_scale=ss)
+    p = w.params
+    p.l2_mode = mode
+    o = oracle_chain(w.hits, w.seg_offsets, w.geometry, p)
+    geo = _geo(B, w.geometry)
+    r = B.process_slice(w.hits, w.seg_offsets, w.run_offsets, geo, _prm(B, p), gather=True)
+    _compare(r, o)
+    assert r.status == 0
+    assert len(o["seeds"]) > 0 and len(o["events"]) > 0
+    tagged = np.nonzero(r.flags & 32)[0]
+    assert r.gathered.tobytes() == r.sorted[tagged].tobytes()
+
+
+@pytest.mark.parametrize("cfg,ts,ss", [(1, 0.05, 1), (3, 0.01, 4 / 64), (4, 0.001, 1)])
+def test_shuffled_input_radix_path(cfg, ts, ss, B, oracle_lib):
+    w = W.make_config(cfg, time_scale=ts, seg_scale=ss)
+    hits, _ = W.shuffled(w)
+    o = oracle_chain(hits, w.seg_offsets, w.geometry, w.params)
+    r = B.process_slice(hits, w.seg_offsets, None, _geo(B, w.geometry), _prm(B, w.params))
+    _compare(r, o)
+
+
+def test_sort_ties_and_extreme_keys(B, oracle_lib):
+    rng = np.random.default_rng(3)
+    n = 50_000
+    h = np.zeros(n, dtype=W.HIT_DTYPE)
+    h["pmt_id"] = rng.integers(0, 84, size=n)
+    h["pad"] = np.arange(n) & 0xFFFF
+    seg = np.array([0, 12345, 12345, n], dtype=np.uint32)
+    geo = _geo(B, W.make_geometry("km3"))
+    prm = B.make_params()
+    for kind in ("ties", "extreme"):
+        h["t_ps"] = rng.integers(0, 40, size=n) if kind == "ties" else rng.integers(-2**62, 2**62, size=n)
+        if kind == "extreme":
+            h["t_ps"][:4] = [-2**63, 2**63 - 1, 0, -1]
+        srt, perm = oracle.sort(h, seg)
+        d_in = B.hits_to_device(h)
+        d_out = torch.empty_like(d_in)
+        d_perm = torch.empty(n, dtype=torch.int32, device="cuda")
+        st = torch.zeros(1, dtype=torch.int32, device="cuda")
+        B.tt_sort_slice(d_in, d_out, d_perm, B.Offsets(seg), None, st)
+        torch.cuda.synchronize()
+        assert B.hits_to_host(d_out).tobytes() == srt.tobytes()
+        assert (d_perm.cpu().numpy().view(np.uint32) == perm).all()
+        # sorted-run path on the same keys: each segment sorted per "PMT" first
+        order = np.concatenate([np.lexsort((np.arange(a, b), h["t_ps"][a:b], h["pmt_id"][a:b])) + a
+                                for a, b in zip(seg[:-1], seg[1:])]) if n else np.zeros(0, dtype=np.int64)
+        hr = h[order]
+        key = np.concatenate([np.full(b - a, k) for k, (a, b) in enumerate(zip(seg[:-1], seg[1:]))]) * 100 + hr["pmt_id"]
+        brk = np.nonzero(np.diff(key))[0] + 1
+        runs = np.concatenate([[0], brk, [n]]).astype(np.uint32)
+        runs = np.unique(np.concatenate([runs, seg])).astype(np.uint32)
+        srt2, perm2 = oracle.sort(hr, seg)
+        d_in = B.hits_to_device(hr)
+        B.tt_sort_slice(d_in, d_out, d_perm, B.Offsets(seg), B.Offsets(runs), st)
+        torch.cuda.synchronize()
+        assert B.hits_to_host(d_out).tobytes() == srt2.tobytes()
+        assert (d_perm.cpu().numpy().view(np.uint32) == perm2).all()
+        assert int(st.item()) == 0
+
+
+def test_status_codes(B, oracle_lib):
+    w = W.make_config(1, time_scale=0.02)
+    geo = _geo(B, w.geometry)
+    prm = _prm(B, w.params)
+    o = oracle_chain(w.hits, w.seg_offsets, w.geometry, w.params)
+    # seed / event capacity too small: true counts reported, prefix valid
+    r = B.process_slice(w.hits, w.seg_offsets, w.run_offsets, geo, prm, seed_cap=3, event_cap=1)
+    assert r.status & B.TT_S_SEED_OVERFLOW and r.n_seeds == len(o["seeds"]) and (r.seeds == o["seeds"][:3]).all()
+    assert (r.flags & 31 == o["flags"] & 31).all()
+    # an unsorted run
+    h = w.hits.copy()
+    a = int(w.run_offsets[3])
+    h[[a, a + 1]] = h[[a + 1, a]]
+    assert h["t_ps"][a] > h["t_ps"][a + 1]
+    r = B.process_slice(h, w.seg_offsets, w.run_offsets, geo, prm)
+    assert r.status & B.TT_S_RUN_UNSORTED
+    # pmt_id out of range on an L1 hit
+    h = w.hits.copy()
+    h["pmt_id"][5] = 500
+    h["charge"][5] = 1000
+    o2 = oracle_chain(h, w.seg_offsets, w.geometry, w.params)
+    r = B.process_slice(h, w.seg_offsets, w.run_offsets, geo, prm)
+    assert (r.status & B.TT_S_BAD_PMT) and (o2["status"] & 8)
+    assert (r.flags == o2["flags"]).all()
+
+
+def test_dense_neighbourhood(B, oracle_lib):
+    """A burst of mutually causal L1 hits: degrees far above 32 (multi-word masks), and above
+    TT_MAX_NEIGHBOURS (TT_S_DENSITY: star bit exact, clique bit left clear, status says so)."""
+    geo_w = W.make_geometry("km3")
+    geo = _geo(B, geo_w)
+    rng = np.random.default_rng(9)
+    for m, expect_density in ((150, False), (300, True)):
+        h = np.zeros(m + 200, dtype=W.HIT_DTYPE)
+        h["pmt_id"] = rng.integers(0, 84, size=len(h))
+        h["floor"] = geo_w.floor[h["pmt_id"]]
+        h["charge"] = 500
+        h["t_ps"][:m] = 1_000_000_000 + np.sort(rng.integers(0, 15_000, size=m))  # all within 15 ns: a clique
+        h["t_ps"][m:] = np.sort(rng.integers(2_000_000_000, 3_000_000_000, size=200))
+        seg = np.array([0, len(h)], dtype=np.uint32)
+        p = W.Params(l2_multiplicity=6)
+        o = oracle_chain(h, seg, geo_w, p)
+        r = B.process_slice(h, seg, None, geo, _prm(B, p))
+        assert ((r.flags & 8) == (o["flags"] & 8)).all()
+        if expect_density:
+            assert r.status & B.TT_S_DENSITY
+            dense = np.arange(len(h)) < m
+            assert ((r.flags & 16)[~dense] == (o["flags"] & 16)[~dense]).all()
+            assert not (r.flags & 16)[dense].any()
+        else:
+            assert r.status == 0
+            assert (r.flags == o["flags"]).all() and (r.seeds == o["seeds"]).all()
+
+
+def test_host_api_matches_device_api(B, oracle_lib):
+    import ctypes
+
+    w = W.make_config(1, time_scale=0.03)
+    geo = _geo(B, w.geometry)
+    prm = _prm(B, w.params)
+    o = oracle_chain(w.hits, w.seg_offsets, w.geometry, w.params)
+    L = B.load()
+    ctx = ctypes.c_void_p(0)
+    n = w.n
+    assert L.tt_host_ctx_create(ctypes.byref(ctx), n, 4, len(w.run_offsets), n, n) == 0
+    srt = np.zeros(n, dtype=B.HIT_DTYPE); fl = np.zeros(n, dtype=np.uint8)
+    seeds = np.zeros(n, dtype=np.uint32); ev = np.zeros(n, dtype=B.EVENT_DTYPE); cnt = np.zeros(3, dtype=np.uint32)
+    vp = lambda a: a.ctypes.data_as(ctypes.c_void_p)
+    seg = np.ascontiguousarray(w.seg_offsets, dtype=np.uint32); runs = np.ascontiguousarray(w.run_offsets, dtype=np.uint32)
+    hin = np.ascontiguousarray(w.hits)
+    rc = L.tt_process_host(ctx, vp(hin), vp(srt), vp(fl), ctypes.c_uint32(n), vp(seg), ctypes.c_uint32(len(seg) - 1),
+                           vp(runs), ctypes.c_uint32(len(runs) - 1), geo.handle, ctypes.byref(prm), vp(seeds), vp(ev),
+                           vp(cnt))
+    assert rc == 0
+    assert srt.tobytes() == o["sorted"].tobytes() and (fl == o["flags"]).all()
+    assert cnt[0] == len(o["seeds"]) and (seeds[: cnt[0]] == o["seeds"]).all()
+    assert cnt[1] == len(o["events"]) and ev[: cnt[1]].tobytes() == o["events"].tobytes()
+    L.tt_host_ctx_destroy(ctx)
