@@ -1,0 +1,346 @@
+#!/usr/bin/env python
+"""bench.py -- sort + trigger + event extraction throughput on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (tt_sort_slice -> tt_trigger_slice -> tt_extract_events
+with INEVT tagging) over one synthetic workload already resident in HBM.  Default workload:
+BASELINE.json configs[4] (100 KM3NeT-It towers, 8400 PMTs, one 200 ms slice, ~92.6 M hits, 1.48 GB --
+larger than the 126 MB L2, so no flush is needed between steps).  N > 1: one process per GPU
+(torchrun), each rank processes its own slice (different seed), no collective on the data path
+("successive time slices are sent to different" trigger nodes): weak scaling.
+
+Prints ONE JSON line (rank 0).  --impl reference times the CPU oracle (oracle/) on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import ctypes
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "hits/s sorted+triggered on 1 B200 (ms per 200 ms slice) and % of HBM roofline"
+ALG_BYTES_PIPELINE = 50  # sort 16 r + 16 w, trigger 16 r + ~2 w
+ALG_BYTES = {"sort": 32, "trig": 18, "ev": 2}
+# bounded oracle sample per config (time_scale, seg_scale): ~10-30 s of single-thread CPU work
+ORACLE_SAMPLE = {0: (1.0, 1.0), 1: (1.0, 1.0), 2: (0.5, 1.0), 3: (1.0, 16 / 64), 4: (0.3, 1.0)}
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def make_workload(cfg: int, rank: int, scale: float):
+    from paper_1411_3968_b200 import workload as W
+
+    if scale == 1.0:
+        return W.make_config(cfg, seed_offset=rank)
+    return W.make_config(cfg, time_scale=scale, seed_offset=rank)
+
+
+def time_oracle(cfg: int, nthreads: int = 1):
+    """The oracle as it stands, single thread, on a bounded sample of config `cfg`."""
+    import oracle
+    from paper_1411_3968_b200 import workload as W
+
+    ts, ss = ORACLE_SAMPLE[cfg]
+    w = W.make_config(cfg, time_scale=ts, seg_scale=ss)
+    g, p = w.geometry, w.params
+    oracle.build()
+    t0 = time.perf_counter()
+    srt, _ = oracle.sort(w.hits, w.seg_offsets)
+    t1 = time.perf_counter()
+    tr = oracle.trigger(srt, w.seg_offsets, g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks,
+                        q_thresh=p.q_thresh, lc_window_ps=p.lc_window_ps, l2_window_ps=p.l2_window_ps,
+                        l2_multiplicity=p.l2_multiplicity, l2_mode=p.l2_mode, event_half_ps=p.event_half_ps)
+    t2 = time.perf_counter()
+    fl = tr.flags.copy()
+    oracle.events(srt, w.seg_offsets, tr.seeds, event_half_ps=p.event_half_ps, flags=fl)
+    t3 = time.perf_counter()
+    sample = (f"cfg{cfg} at time_scale={ts}, seg_scale={ss}: {w.n} hits; sort {1e3 * (t1 - t0):.0f} ms, "
+              f"trigger {1e3 * (t2 - t1):.0f} ms, events {1e3 * (t3 - t2):.0f} ms")
+    return w.n, t3 - t0, sample, w.name
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    for _ in range(args.warmup):
+        pass  # the oracle has no warm state worth priming beyond the build
+    times, n, sample, name = [], 0, "", ""
+    for _ in range(max(1, args.steps)):
+        n, dt, sample, name = time_oracle(args.config)
+        times.append(dt)
+        if sum(times) > 150:
+            break
+    dt = float(np.mean(times))
+    v = n / dt
+    slices = {0: 1, 1: 1, 2: 5, 3: 64, 4: 1}[args.config]
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": "hits/s", "n_gpus": args.gpus, "steps": len(times),
+        "warmup": args.warmup, "ms_per_step": 1e3 * dt, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+        "config": {"workload": name, "sample": sample, "slices_full_config": slices},
+        "cpu_baseline": {"value": v, "unit": "hits/s", "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": "hits/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def run_ours(args):
+    import torch
+
+    from paper_1411_3968_b200 import binding as B
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.load()
+    w = make_workload(args.config, rank, args.scale)
+    n = w.n
+    g = w.geometry
+    geo = B.Geometry(g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks)
+    p = w.params
+    prm = B.make_params(p.q_thresh, p.lc_window_ps, p.l2_window_ps, p.l2_multiplicity, p.l2_mode, p.event_half_ps)
+    seg, runs = B.Offsets(w.seg_offsets), B.Offsets(w.run_offsets)
+    d_in = B.hits_to_device(w.hits)
+    d_out = torch.empty_like(d_in)
+    seed_cap = event_cap = max(n // 4, 1024)
+    d_flags = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    d_seeds = torch.zeros(seed_cap, dtype=torch.int32, device="cuda")
+    d_ev = torch.zeros((event_cap, 4), dtype=torch.int64, device="cuda")
+    d_cnt = torch.zeros(4, dtype=torch.int32, device="cuda")  # n_seeds, n_events, status, spare
+    d_ns, d_ne, d_st = d_cnt[0:1], d_cnt[1:2], d_cnt[2:3]
+    ws = {}
+
+    def step():
+        d_cnt.zero_()
+        ws["s"] = B.tt_sort_slice(d_in, d_out, None, seg, runs, d_st, ws.get("s"))
+        ws["t"] = B.tt_trigger_slice(d_out, seg, geo, prm, d_flags, d_seeds, d_ns, d_st, ws.get("t"))
+        ws["e"] = B.tt_extract_events(d_out, seg, d_seeds, d_ns, prm, d_ev, d_ne, d_flags, None, None, d_st, ws.get("e"))
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    counts = d_cnt.cpu().numpy().view(np.uint32)
+    n_seeds, n_events, status = int(counts[0]), int(counts[1]), int(counts[2])
+    l1_frac = float((d_flags & 4).ne(0).float().mean().item())
+    inevt_frac = float((d_flags & 32).ne(0).float().mean().item())
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    B.prof_enable(True)
+    l0 = B.launch_count()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    launches = B.launch_count() - l0
+    ms_total = e0.elapsed_time(e1)
+    stages = B.prof_read()
+    B.prof_enable(False)
+    clocks = sampler.stop()
+    ms_step = ms_total / args.steps
+    if dist is not None:
+        t = torch.tensor([ms_step], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_step = float(t.item())
+        tn = torch.tensor([n], device="cuda", dtype=torch.float64)
+        dist.all_reduce(tn, op=dist.ReduceOp.SUM)
+        n_total = int(tn.item())
+    else:
+        n_total = n
+    value = n_total / (ms_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (device time from the stage events of the timed steps) ----
+    peak, peak_src = peaks()
+    per_stage = {k: v[0] / args.steps for k, v in stages.items()}  # ms per step
+    dom = max(per_stage, key=per_stage.get) if per_stage else None
+    roof = None
+    if dom:
+        launches_dom = stages[dom][1] / args.steps
+        alg = ALG_BYTES[dom.split(".")[0]] * n  # bytes the whole stage family must move once per step
+        # a stage that runs several times per step (radix passes) still has to move the algorithmic bytes once
+        dur_ms = per_stage[dom]
+        ach = alg / (dur_ms * 1e-3) / 1e9
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            try:
+                traffic = json.load(open(tp)).get(f"cfg{args.config}", {}).get(dom)
+            except Exception:
+                traffic = None
+        roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": traffic, "peak_source": peak_src, "alg_bytes_per_launch": alg / max(launches_dom, 1),
+                "launches_per_step": launches_dom, "kernel_ms_per_step": dur_ms,
+                "share_of_step": dur_ms / (ms_total / args.steps)}
+    pipe_ach = ALG_BYTES_PIPELINE * n / (ms_total / args.steps * 1e-3) / 1e9
+
+    # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
+    e2e = None
+    if not args.no_e2e:
+        L = B.load()
+        ctx = ctypes.c_void_p(0)
+        rc = L.tt_host_ctx_create(ctypes.byref(ctx), ctypes.c_uint32(n), ctypes.c_uint32(seg.count),
+                                  ctypes.c_uint32(runs.count), ctypes.c_uint32(seed_cap), ctypes.c_uint32(event_cap))
+        if rc != 0:
+            raise SystemExit(f"tt_host_ctx_create failed: {rc}")
+        h_in = torch.from_numpy(w.hits.view(np.int64).reshape(-1, 2)).pin_memory()
+        h_flags = torch.empty(n, dtype=torch.uint8).pin_memory()
+        h_seeds = torch.empty(seed_cap, dtype=torch.int32).pin_memory()
+        h_ev = torch.empty((event_cap, 4), dtype=torch.int64).pin_memory()
+        h_cnt = np.zeros(4, dtype=np.uint32)
+        vp = ctypes.c_void_p
+
+        def host_step():
+            rc = L.tt_process_host(ctx, vp(h_in.data_ptr()), vp(0), vp(h_flags.data_ptr()), ctypes.c_uint32(n),
+                                   seg.h.ctypes.data_as(vp), ctypes.c_uint32(seg.count), runs.h.ctypes.data_as(vp),
+                                   ctypes.c_uint32(runs.count), geo.handle, ctypes.byref(prm), vp(h_seeds.data_ptr()),
+                                   vp(h_ev.data_ptr()), h_cnt.ctypes.data_as(vp))
+            if rc != 0:
+                raise SystemExit(f"tt_process_host failed: {rc}")
+
+        host_step()
+        barrier()
+        k2 = max(1, min(args.steps, 5))
+        t0 = time.perf_counter()
+        for _ in range(k2):
+            host_step()
+        dt = (time.perf_counter() - t0) / k2
+        if dist is not None:
+            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        ns, ne = int(min(h_cnt[0], seed_cap)), int(min(h_cnt[1], event_cap))
+        e2e = {"value": n_total / dt, "unit": "hits/s", "ms_per_step": 1e3 * dt,
+               "h2d_bytes_per_step": int(16 * n + 4 * (seg.count + 1) + 4 * (runs.count + 1)),
+               "d2h_bytes_per_step": int(n + 4 * ns + 32 * ne + 12),
+               "api": "tt_process_host (pinned host buffers; returns flags, seeds, events)"}
+        assert int(h_cnt[0]) == n_seeds and int(h_cnt[1]) == n_events, "host path disagrees with device path"
+        L.tt_host_ctx_destroy(ctx)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        on, odt, sample, _ = time_oracle(args.config)
+        cpu = {"value": on / odt, "unit": "hits/s", "cores": 1, "kind": "oracle", "sample": sample}
+
+    if rank == 0:
+        slices = w.n_slices
+        out = {
+            "metric": METRIC, "value": value, "unit": "hits/s", "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int64", "data": "synthetic",
+            "config": {"workload": w.name, "hits_per_rank": n, "slices_per_step": slices,
+                       "ms_per_200ms_slice": ms_step / slices, "l2_flush": "inputs larger than L2 (16 B x n)"
+                       if 16 * n > 130e6 else "inputs fit in L2: not flushed (launch-bound config)",
+                       "n_seeds": n_seeds, "n_events": n_events, "status": status, "l1_fraction": l1_frac,
+                       "inevt_fraction": inevt_frac, "parallelism": f"slice-per-gpu x{world}"},
+            "clocks": clocks, "gpu_launches": int(launches),
+            "roofline": roof,
+            "pipeline_roofline": {"alg_bytes_per_hit": ALG_BYTES_PIPELINE, "achieved": pipe_ach, "peak": peak,
+                                  "unit": "GB/s", "frac": pipe_ach / peak},
+            "stages_ms_per_step": {k: round(v, 5) for k, v in sorted(per_stage.items())},
+            "e2e": e2e, "cpu_baseline": cpu,
+        }
+        print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--scale", type=float, default=1.0, help="time_scale < 1 shrinks the workload (debugging only)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -140,6 +140,14 @@ int tt_process_host(tt_host_ctx* c, const tt_hit* h_in, tt_hit* h_sorted, uint8_
                     uint32_t n_runs, const tt_geometry* g, const tt_params* p, uint32_t* h_seeds,
                     tt_event* h_events, uint32_t* h_counts);
 
+/* Instrumentation (not on the data path).  tt_launch_count: kernels launched by this library in
+ * this process so far.  tt_prof_enable(1) makes every stage boundary inside the hot calls record a
+ * CUDA event on the caller's stream; after synchronising, tt_prof_read writes one line per stage,
+ * "name total_ms count", into buf (returns bytes written, < 0 on error); tt_prof_enable(0) stops. */
+uint64_t tt_launch_count(void);
+int tt_prof_enable(int on);
+int tt_prof_read(char* buf, size_t cap);
+
 /* Library version / build string (static storage). */
 const char* tt_version(void);
 

@@ -22,7 +22,8 @@ TT_OK, TT_E_INVAL, TT_E_CUDA, TT_E_WORKSPACE = 0, -1, -2, -3
 TT_S_SEED_OVERFLOW, TT_S_EVENT_OVERFLOW, TT_S_RUN_UNSORTED, TT_S_BAD_PMT, TT_S_DENSITY = 1, 2, 4, 8, 16
 
 EXPORTS = ["tt_version", "tt_geometry_create", "tt_geometry_destroy", "tt_sort_slice", "tt_trigger_slice",
-           "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host"]
+           "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host", "tt_launch_count",
+           "tt_prof_enable", "tt_prof_read"]
 
 HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
 EVENT_DTYPE = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
@@ -61,8 +62,30 @@ def load(build: bool = True):
         L.tt_version.restype = ctypes.c_char_p
         for name in EXPORTS[1:]:
             getattr(L, name).restype = ctypes.c_int
+        L.tt_launch_count.restype = ctypes.c_uint64
         _lib = L
     return _lib
+
+
+def launch_count() -> int:
+    return int(load().tt_launch_count())
+
+
+def prof_enable(on: bool):
+    load().tt_prof_enable(c_i32(1 if on else 0))
+
+
+def prof_read() -> dict[str, tuple[float, int]]:
+    """{stage: (total ms, count)} since prof_enable(True); synchronise first."""
+    buf = ctypes.create_string_buffer(1 << 16)
+    nb = load().tt_prof_read(buf, c_sz(len(buf)))
+    if nb < 0:
+        raise TTError("tt_prof_read failed")
+    out = {}
+    for line in buf.raw[:nb].decode().splitlines():
+        name, ms, cnt = line.split()
+        out[name] = (float(ms), int(cnt))
+    return out
 
 
 def _check(rc: int, what: str):

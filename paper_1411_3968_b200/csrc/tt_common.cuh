@@ -22,6 +22,13 @@ namespace tt {
 
 constexpr int kSMs = 148;  // B200
 
+// ---- launch counter and stage profiler (tt_prof.cu) ------------------------------------------------
+void count_launch();                                // every kernel launch of the library goes through TT_K
+void prof_mark(cudaStream_t s, const char* name);   // no-op unless tt_prof_enable(1): records an event that
+                                                    // opens stage `name` (and closes the previous one)
+void prof_end(cudaStream_t s);                      // closes the current stage
+#define TT_K(k) tt::count_launch(), k
+
 struct tt_geometry_dev {  // device view of the causality table
     const int32_t* pair_block;  // [n_tower*n_tower]
     const int32_t* blocks;      // [n_blocks][ppt][ppt]

@@ -282,22 +282,26 @@ extern "C" int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint3
     const SegCtx sc{d_seg_offsets, n_seg, n};
     const uint64_t twoH = 2ull * (uint64_t)p->event_half_ps;
     const uint4* hits = (const uint4*)d_sorted;
-    ev_count_kernel<<<kEvBlocks, kEvThreads, 0, s>>>(hits, d_seeds, d_n_seeds, seed_cap, sc, twoH, plan.cnt);
-    ev_scan_kernel<<<1, 1024, 0, s>>>(plan.cnt, kEvBlocks, d_n_events, event_cap, d_status);
-    ev_write_kernel<<<kEvBlocks, kEvThreads, 0, s>>>(hits, d_seeds, d_n_seeds, seed_cap, sc, twoH, p->event_half_ps,
+    prof_mark(s, "ev.merge");
+    TT_K(ev_count_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(hits, d_seeds, d_n_seeds, seed_cap, sc, twoH, plan.cnt);
+    TT_K(ev_scan_kernel)<<<1, 1024, 0, s>>>(plan.cnt, kEvBlocks, d_n_events, event_cap, d_status);
+    TT_K(ev_write_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(hits, d_seeds, d_n_seeds, seed_cap, sc, twoH, p->event_half_ps,
                                                      plan.cnt, d_events, event_cap);
-    ev_fix_kernel<<<kSMs, 256, 0, s>>>(d_events, d_n_events, event_cap);
+    TT_K(ev_fix_kernel)<<<kSMs, 256, 0, s>>>(d_events, d_n_events, event_cap);
     if (d_gather || d_n_gathered) {
-        len_count_kernel<<<kEvBlocks, kEvThreads, 0, s>>>(d_events, d_n_events, event_cap, plan.cnt2);
-        len_scan_kernel<<<1, 1024, 0, s>>>(plan.cnt2, kEvBlocks, d_n_gathered ? d_n_gathered : plan.n_gathered_dummy);
+        prof_mark(s, "ev.gather_scan");
+        TT_K(len_count_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(d_events, d_n_events, event_cap, plan.cnt2);
+        TT_K(len_scan_kernel)<<<1, 1024, 0, s>>>(plan.cnt2, kEvBlocks, d_n_gathered ? d_n_gathered : plan.n_gathered_dummy);
         if (d_gather)
-            len_write_kernel<<<kEvBlocks, kEvThreads, 0, s>>>(d_events, d_n_events, event_cap, plan.cnt2, plan.goff);
+            TT_K(len_write_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(d_events, d_n_events, event_cap, plan.cnt2, plan.goff);
     }
     if (d_flags || d_gather) {
         const uint32_t nb = div_up(n, kTagThreads * kTagPer);
-        tag_gather_kernel<<<nb, kTagThreads, 0, s>>>(hits, n, d_events, d_n_events, event_cap, d_flags,
+        prof_mark(s, "ev.tag_gather");
+        TT_K(tag_gather_kernel)<<<nb, kTagThreads, 0, s>>>(hits, n, d_events, d_n_events, event_cap, d_flags,
                                                      (uint4*)d_gather, plan.goff);
     }
+    prof_end(s);
     TT_LAUNCH_OK();
     return TT_OK;
 }

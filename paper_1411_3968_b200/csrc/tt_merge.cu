@@ -26,7 +26,8 @@ size_t merge_ws_bytes(uint32_t n, const uint32_t*, uint32_t, const uint32_t*, ui
 int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, const uint32_t* d_seg_offsets,
                     const uint32_t*, uint32_t n_seg, const uint32_t* d_run_offsets, const uint32_t*, uint32_t n_runs,
                     void* d_ws, int32_t* d_status, cudaStream_t s) {
-    run_check_kernel<<<div_up(n, 256), 256, 0, s>>>((const uint4*)d_in, n, d_run_offsets, n_runs, d_status);
+    prof_mark(s, "sort.run_check");
+    TT_K(run_check_kernel)<<<div_up(n, 256), 256, 0, s>>>((const uint4*)d_in, n, d_run_offsets, n_runs, d_status);
     return radix_sort(d_in, d_out, d_perm, n, d_seg_offsets, n_seg, d_ws, s);
 }
 }  // namespace tt

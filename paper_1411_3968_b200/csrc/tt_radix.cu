@@ -177,20 +177,26 @@ int radix_sort(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, 
     RadixPlan p;
     radix_plan(a, n, p);
     const uint32_t nb256 = div_up(n, 256);
-    radix_extract_kernel<<<nb256, 256, 0, s>>>((const uint4*)d_in, p.keys0, p.idx0, n, p.st);
+    prof_mark(s, "sort.radix_extract");
+    TT_K(radix_extract_kernel)<<<nb256, 256, 0, s>>>((const uint4*)d_in, p.keys0, p.idx0, n, p.st);
     int seg_passes = 0;
     for (uint32_t v = n_seg - 1; v; v >>= 8) ++seg_passes;
     for (int pass = 0; pass < 8 + seg_passes; ++pass) {
-        radix_hist_kernel<<<p.nblocks, kRThreads, 0, s>>>(p.keys0, p.keys1, p.idx0, p.idx1, n, pass, d_seg_offsets,
+        prof_mark(s, "sort.radix_hist");
+        TT_K(radix_hist_kernel)<<<p.nblocks, kRThreads, 0, s>>>(p.keys0, p.keys1, p.idx0, p.idx1, n, pass, d_seg_offsets,
                                                           n_seg, p.st, p.hist, p.nblocks);
+        prof_mark(s, "sort.radix_scan");
         int rc = exclusive_scan_u32(p.hist, p.hist, 256u * p.nblocks, p.scan_scratch, nullptr, s);
         if (rc != TT_OK) return rc;
-        radix_decide_kernel<<<1, 256, 0, s>>>(p.hist, p.nblocks, n, p.st);
-        radix_scatter_kernel<<<p.nblocks, kRThreads, 0, s>>>(p.keys0, p.keys1, p.idx0, p.idx1, n, pass,
+        TT_K(radix_decide_kernel)<<<1, 256, 0, s>>>(p.hist, p.nblocks, n, p.st);
+        prof_mark(s, "sort.radix_scatter");
+        TT_K(radix_scatter_kernel)<<<p.nblocks, kRThreads, 0, s>>>(p.keys0, p.keys1, p.idx0, p.idx1, n, pass,
                                                              d_seg_offsets, n_seg, p.st, p.hist, p.nblocks);
-        radix_flip_kernel<<<1, 1, 0, s>>>(p.st);
+        TT_K(radix_flip_kernel)<<<1, 1, 0, s>>>(p.st);
     }
-    radix_gather_kernel<<<nb256, 256, 0, s>>>((const uint4*)d_in, (uint4*)d_out, d_perm, p.idx0, p.idx1, p.st, n);
+    prof_mark(s, "sort.radix_gather");
+    TT_K(radix_gather_kernel)<<<nb256, 256, 0, s>>>((const uint4*)d_in, (uint4*)d_out, d_perm, p.idx0, p.idx1, p.st, n);
+    prof_end(s);
     TT_LAUNCH_OK();
     return TT_OK;
 }

@@ -73,17 +73,17 @@ int exclusive_scan_u32(const uint32_t* in, uint32_t* out, uint32_t n, uint32_t* 
     }
     const uint32_t nb1 = div_up(n, kScanTile);
     uint32_t* sums1 = scratch;
-    scan_reduce_kernel<<<nb1, kScanThreads, 0, s>>>(in, sums1, n);
+    TT_K(scan_reduce_kernel)<<<nb1, kScanThreads, 0, s>>>(in, sums1, n);
     if (nb1 <= 8192) {
-        scan_small_kernel<<<1, 1024, 0, s>>>(sums1, nb1, total);
+        TT_K(scan_small_kernel)<<<1, 1024, 0, s>>>(sums1, nb1, total);
     } else {
         const uint32_t nb2 = div_up(nb1, kScanTile);
         uint32_t* sums2 = scratch + nb1;
-        scan_reduce_kernel<<<nb2, kScanThreads, 0, s>>>(sums1, sums2, nb1);
-        scan_small_kernel<<<1, 1024, 0, s>>>(sums2, nb2, total);
-        scan_apply_kernel<<<nb2, kScanThreads, 0, s>>>(sums1, sums1, sums2, nb1);
+        TT_K(scan_reduce_kernel)<<<nb2, kScanThreads, 0, s>>>(sums1, sums2, nb1);
+        TT_K(scan_small_kernel)<<<1, 1024, 0, s>>>(sums2, nb2, total);
+        TT_K(scan_apply_kernel)<<<nb2, kScanThreads, 0, s>>>(sums1, sums1, sums2, nb1);
     }
-    scan_apply_kernel<<<nb1, kScanThreads, 0, s>>>(in, out, sums1, n);
+    TT_K(scan_apply_kernel)<<<nb1, kScanThreads, 0, s>>>(in, out, sums1, n);
     TT_LAUNCH_OK();
     return TT_OK;
 }

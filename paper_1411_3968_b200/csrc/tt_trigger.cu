@@ -392,18 +392,24 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
                                         (int)(sizeof(L2Smem) * kL2Warps)));
         attr_done = true;
     }
-    l1_flags_kernel<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,
+    prof_mark(s, "trig.l1_flags");
+    TT_K(l1_flags_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,
                                                      (uint64_t)p->lc_window_ps, p->q_thresh, d_flags, plan.blk_cnt);
+    prof_mark(s, "trig.l1_scan");
     int rc = exclusive_scan_u32(plan.blk_cnt, plan.blk_cnt, plan.nblk, plan.scan_scratch, plan.m_total, s);
     if (rc != TT_OK) return rc;
-    l1_compact_kernel<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1);
-    l2_kernel<<<kSMs * 8, kL2Warps * 32, sizeof(L2Smem) * kL2Warps, s>>>(
+    prof_mark(s, "trig.l1_compact");
+    TT_K(l1_compact_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1);
+    prof_mark(s, "trig.l2");
+    TT_K(l2_kernel)<<<kSMs * 8, kL2Warps * 32, sizeof(L2Smem) * kL2Warps, s>>>(
         plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps, p->l2_multiplicity,
         p->l2_mode, d_flags, plan.l2bit, d_status);
-    seed_count_kernel<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.m_total, plan.seed_cnt);
-    count_scan_kernel<<<1, 1024, 0, s>>>(plan.seed_cnt, kSeedBlocks, d_n_seeds, seed_cap, TT_S_SEED_OVERFLOW, d_status);
-    seed_write_kernel<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.l1, plan.m_total, plan.seed_cnt, d_seeds,
+    prof_mark(s, "trig.seeds");
+    TT_K(seed_count_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.m_total, plan.seed_cnt);
+    TT_K(count_scan_kernel)<<<1, 1024, 0, s>>>(plan.seed_cnt, kSeedBlocks, d_n_seeds, seed_cap, TT_S_SEED_OVERFLOW, d_status);
+    TT_K(seed_write_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.l1, plan.m_total, plan.seed_cnt, d_seeds,
                                                            seed_cap);
+    prof_end(s);
     TT_LAUNCH_OK();
     return TT_OK;
 }
