@@ -1,33 +1,565 @@
-// tt_merge.cu -- sort of P concatenated, individually time-ordered runs (the per-PMT streams,
-// "our data ... is time-ordered for single PMT").
-// v0: verifies the runs and falls through to the general radix path.
+// tt_merge.cu -- time sort of P concatenated, individually time-ordered runs (the per-PMT streams:
+// PAPER.md:23 "merges together the 16 PMT data streams", "our data ... is time-ordered
+// for single PMT"; north_star: "a merge of the per-PMT time-ordered streams").
+//
+// One pass per level: the runs of a group (<= fan-in F consecutive runs of one segment) are cut at
+// uniform time boundaries into tiles of ~3.5 k hits (binary search of every run at every boundary),
+// one CTA stages the <= F short run pieces of its tile in shared memory (run-major = input order),
+// ranks them with a counting sort on fine time buckets (shared-memory atomics for the histogram,
+// exact (time, input order) comparison inside a bucket, so the result is the stable order), and
+// writes the tile with coalesced 16-byte stores.  P <= 512 runs per segment: one level (32 B/hit of
+// HBM traffic).  More runs (cfg4: 8400): ceil(log_512 P) levels with fan-in ceil(P^(1/levels)).
+//
+// The plan (groups, tile counts, split tables) is computed on the device from the offsets, so the
+// call stays asynchronous and allocation-free; the host mirrors the same integer arithmetic only to
+// size grids and the workspace.
+//
+// Robustness: a tile whose pieces hold more than kCap hits (non-uniform density, massive ties) is
+// swept in time order in chunks of <= kCap hits found by bisection on the key; a single timestamp
+// with more than kCap hits is emitted as the run-major concatenation (which is the stable order).
+#include <vector>
+
 #include "tt_common.cuh"
 
 namespace tt {
-size_t radix_ws_bytes(uint32_t n);
-int radix_sort(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, const uint32_t* d_seg_offsets,
-               uint32_t n_seg, void* d_ws, cudaStream_t s);
 
-// run r with off[r] <= i < off[r+1]
-__global__ void __launch_bounds__(256) run_check_kernel(const uint4* __restrict__ hits, uint32_t n,
-                                                        const uint32_t* __restrict__ run_off, uint32_t n_runs,
-                                                        int32_t* __restrict__ status) {
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    bool bad = false;
-    if (i > 0 && i < n) {
-        const uint32_t r = find_segment(run_off, n_runs, i);
-        if (__ldg(run_off + r) != i) bad = hit_time(__ldg(hits + i)) < hit_time(__ldg(hits + i - 1));
-    }
-    if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(status, TT_S_RUN_UNSORTED);
+constexpr int kMThreads = 512;
+constexpr int kCap = 4096;                    // hits staged per chunk
+constexpr int kMItems = kCap / kMThreads;     // 8
+constexpr uint32_t kTileTarget = 3584;        // expected hits per tile (0.875 kCap)
+constexpr int kMaxFan = 512;                  // runs per group
+
+struct LevelDev {
+    const uint32_t* roff;    // [R+1] run offsets of this level
+    uint32_t* gfirst;        // [G+1] first run of each group
+    uint32_t* tbase;         // [G+1] exclusive prefix of tiles per group
+    uint32_t* sbase;         // [G+1] exclusive prefix of split-table entries per group ((tiles+1) * K)
+    uint64_t* gT0;           // [G] smallest key of the group
+    uint64_t* gDT;           // [G] tile width in key units (>= 1)
+    uint32_t* splits;        // split table
+    uint32_t* roff_next;     // [G+1] run offsets of the next level (= group boundaries)
+    uint32_t R, G, F;
+};
+
+__host__ __device__ inline uint32_t tiles_for(uint32_t n_g) { return (n_g + kTileTarget - 1) / kTileTarget; }
+
+__device__ __forceinline__ uint64_t key_at(const uint4* __restrict__ hits, uint32_t i) {
+    return key_of(hit_time(__ldg(hits + i)));
 }
 
-size_t merge_ws_bytes(uint32_t n, const uint32_t*, uint32_t, const uint32_t*, uint32_t) { return radix_ws_bytes(n); }
+// ---- plan step 1: groups.  Segment s owns the runs [lb(roff, seg[s]), lb(roff, seg[s+1])) and is cut into
+// consecutive groups of F runs.  One block; loops over segments with a running carry.
+__global__ void __launch_bounds__(1024) merge_groups_kernel(LevelDev lv, const uint32_t* __restrict__ seg_off,
+                                                            uint32_t n_seg) {
+    __shared__ uint32_t sm[33];
+    uint32_t carry = 0;
+    for (uint32_t base = 0; base < n_seg; base += 1024) {
+        const uint32_t s = base + threadIdx.x;
+        uint32_t r0 = 0, r1 = 0, ng = 0;
+        if (s < n_seg) {
+            const uint32_t a = seg_off[s], b = seg_off[s + 1];
+            uint32_t lo = 0, hi = lv.R;  // first run index with roff[r] >= a
+            while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (lv.roff[mid] < a) lo = mid + 1; else hi = mid; }
+            r0 = lo;
+            lo = r0; hi = lv.R;
+            if (s + 1 == n_seg) r1 = lv.R;
+            else { while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (lv.roff[mid] < b) lo = mid + 1; else hi = mid; } r1 = lo; }
+            ng = (r1 - r0 + lv.F - 1) / lv.F;
+        }
+        uint32_t total;
+        const uint32_t ex = block_exclusive_scan(ng, sm, &total);
+        for (uint32_t q = 0; q < ng; ++q) lv.gfirst[carry + ex + q] = r0 + q * lv.F;
+        carry += total;
+    }
+    if (threadIdx.x == 0) lv.gfirst[carry] = lv.R;  // carry == G
+}
+
+// ---- plan step 2: per group: hit count, tile count, key range, tile width; prefixes.  One block,
+// one warp per group (lanes over the group's runs).
+__global__ void __launch_bounds__(1024) merge_setup_kernel(LevelDev lv, const uint4* __restrict__ hits, uint32_t n) {
+    __shared__ uint32_t sm[33];
+    const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // pass A: per-group ranges (warp per group)
+    for (uint32_t g = warp; g < lv.G; g += 32) {
+        const uint32_t r0 = lv.gfirst[g], r1 = lv.gfirst[g + 1];
+        uint64_t kmin = ~0ull, kmax = 0;
+        for (uint32_t r = r0 + lane; r < r1; r += 32) {
+            const uint32_t a = lv.roff[r], b = lv.roff[r + 1];
+            if (b > a) {
+                const uint64_t k0 = key_at(hits, a), k1 = key_at(hits, b - 1);
+                kmin = k0 < kmin ? k0 : kmin;
+                kmax = k1 > kmax ? k1 : kmax;
+            }
+        }
+#pragma unroll
+        for (int d = 16; d; d >>= 1) {
+            const uint64_t o0 = __shfl_xor_sync(0xffffffffu, kmin, d), o1 = __shfl_xor_sync(0xffffffffu, kmax, d);
+            kmin = o0 < kmin ? o0 : kmin;
+            kmax = o1 > kmax ? o1 : kmax;
+        }
+        if (lane == 0) {
+            const uint32_t n_g = lv.roff[r1] - lv.roff[r0];
+            const uint32_t nt = tiles_for(n_g);
+            lv.gT0[g] = kmin;
+            lv.gDT[g] = nt ? (kmax >= kmin ? (kmax - kmin) / nt + 1 : 1) : 1;
+            lv.roff_next[g] = lv.roff[r0];
+        }
+    }
+    if (threadIdx.x == 0) lv.roff_next[lv.G] = n;
+    __syncthreads();
+    // pass B: prefixes of tiles and split entries
+    uint32_t carry_t = 0, carry_s = 0;
+    for (uint32_t base = 0; base < lv.G; base += 1024) {
+        const uint32_t g = base + threadIdx.x;
+        uint32_t nt = 0, ns = 0;
+        if (g < lv.G) {
+            const uint32_t r0 = lv.gfirst[g], r1 = lv.gfirst[g + 1];
+            nt = tiles_for(lv.roff[r1] - lv.roff[r0]);
+            ns = nt ? (nt + 1) * (r1 - r0) : 0;
+        }
+        uint32_t tt_, ts_;
+        const uint32_t et = block_exclusive_scan(nt, sm, &tt_);
+        const uint32_t es = block_exclusive_scan(ns, sm, &ts_);
+        if (g < lv.G) { lv.tbase[g] = carry_t + et; lv.sbase[g] = carry_s + es; }
+        carry_t += tt_;
+        carry_s += ts_;
+    }
+    if (threadIdx.x == 0) { lv.tbase[lv.G] = carry_t; lv.sbase[lv.G] = carry_s; }
+}
+
+// ---- plan step 3: split table.  Entry (g, k, j): first index of run j of group g with key >= T0 + k*DT
+// (k = 0: run start; k = tiles: run end).
+__global__ void __launch_bounds__(256) merge_partition_kernel(LevelDev lv, const uint4* __restrict__ hits,
+                                                              uint32_t total) {
+    const uint32_t id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= total) return;
+    uint32_t lo = 0, hi = lv.G;  // group with sbase[g] <= id < sbase[g+1]
+    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (lv.sbase[mid] <= id) lo = mid; else hi = mid; }
+    const uint32_t g = lo;
+    const uint32_t r0 = lv.gfirst[g], K = lv.gfirst[g + 1] - r0;
+    const uint32_t local = id - lv.sbase[g];
+    const uint32_t k = local / K, j = local - k * K;
+    const uint32_t nt = lv.tbase[g + 1] - lv.tbase[g];
+    uint32_t a = lv.roff[r0 + j], b = lv.roff[r0 + j + 1];
+    uint32_t res;
+    if (k == 0) res = a;
+    else if (k >= nt) res = b;
+    else {
+        const uint64_t T0 = lv.gT0[g], DT = lv.gDT[g];
+        const uint64_t add = (uint64_t)k * DT;  // k < 2^20, DT <= 2^64 / nt: no overflow of the product
+        const uint64_t T = T0 + add < T0 ? ~0ull : T0 + add;
+        while (a < b) { const uint32_t mid = a + ((b - a) >> 1); if (key_at(hits, mid) < T) a = mid + 1; else b = mid; }
+        res = a;
+    }
+    lv.splits[id] = res;
+}
+
+// ---- the tile kernel ---------------------------------------------------------------------------------
+struct MergeSmem {
+    uint4 tile[kCap];             // staged records, run-major                       64 KB
+    uint32_t cnt[kCap];           // bucket counters -> exclusive starts             16 KB
+    uint16_t list[kCap];          // bucket member lists (tile-local element ids)     8 KB
+    uint16_t inv[kCap];           // inv[rank] = element id                           8 KB
+    uint32_t segstart[kMaxFan + 1];  // tile-local start of every run piece
+    uint32_t cur[kMaxFan];        // absolute index of the next unprocessed hit of every run
+    uint32_t end[kMaxFan];        // absolute end of every run piece of this tile
+    uint32_t mid[kMaxFan];        // scratch: chunk ends
+    uint32_t scan[33];
+    uint64_t red64[2 * (kMThreads / 32)];
+};
+
+__device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* sm) {
+    uint32_t total;
+    block_exclusive_scan(v, sm, &total);
+    return total;
+}
+
+// Sort the chunk [cur_j, mid_j) over the runs j < K (<= kCap hits in total) and write it at out_base.
+// Keys of the chunk lie in [Ta, Ta + width).  Returns the chunk size (uniform over the block).
+template <bool kPerm>
+__device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint4* __restrict__ out, uint32_t K,
+                               const uint32_t* chunk_end, uint64_t Ta, uint64_t width, uint32_t out_base,
+                               const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out, bool check_runs,
+                               const uint32_t* __restrict__ run_begin, int32_t* __restrict__ status) {
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    // tile-local piece starts
+    {
+        const uint32_t len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
+        uint32_t total;
+        const uint32_t ex = block_exclusive_scan(len, sm.scan, &total);
+        if (tid < K) sm.segstart[tid] = ex;
+        if (tid == 0) sm.segstart[K] = total;
+    }
+    for (uint32_t b = tid; b < (uint32_t)kCap; b += kMThreads) sm.cnt[b] = 0;
+    __syncthreads();
+    const uint32_t count = sm.segstart[K];
+    // stage the pieces: one warp per run, lanes over consecutive records (coalesced 16-byte loads)
+    bool unsorted = false;
+    for (uint32_t j = warp; j < K; j += kMThreads / 32) {
+        const uint32_t a = sm.cur[j], s0 = sm.segstart[j], len = sm.segstart[j + 1] - s0;
+        uint64_t carry_key = 0;
+        bool have_carry = false;
+        if (check_runs && len && a > run_begin[j]) { carry_key = key_at(in, a - 1); have_carry = true; }
+        for (uint32_t p0 = 0; p0 < len; p0 += 32) {
+            const uint32_t p = p0 + lane;
+            uint4 v = make_uint4(0, 0, 0, 0);
+            if (p < len) { v = __ldg(in + a + p); sm.tile[s0 + p] = v; }
+            if (check_runs) {
+                const uint64_t k = key_of(hit_time(v));
+                uint64_t prev = __shfl_up_sync(0xffffffffu, k, 1);
+                bool has_prev = lane > 0;
+                if (lane == 0) { prev = carry_key; has_prev = have_carry; }
+                if (p < len && has_prev && prev > k) unsorted = true;
+                carry_key = __shfl_sync(0xffffffffu, k, 31);
+                have_carry = true;
+            }
+        }
+    }
+    if (check_runs && __syncthreads_or(unsorted) && tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
+    __syncthreads();
+    // bucket function: monotone map of (key - Ta) in [0, width) onto [0, kCap)
+    int pre = 0;
+    while ((width >> pre) > 0xFFFFFFFFull) ++pre;
+    const uint32_t wp = (uint32_t)(width >> pre);
+    const bool direct = wp <= (uint32_t)kCap;
+    const uint32_t scale = direct ? 0u : (uint32_t)(((uint64_t)kCap << 32) / wp);
+    uint32_t bk[kMItems], slot[kMItems];
+#pragma unroll
+    for (int i = 0; i < kMItems; ++i) {
+        const uint32_t e = tid + i * kMThreads;
+        bk[i] = 0; slot[i] = 0;
+        if (e < count) {
+            const uint64_t key = key_of(hit_time(sm.tile[e]));
+            uint64_t dt = key - Ta;
+            if (key < Ta) dt = 0;
+            if (dt >= width) dt = width - 1;
+            const uint32_t d = (uint32_t)(dt >> pre);
+            uint32_t b = direct ? d : __umulhi(d, scale);
+            if (b >= (uint32_t)kCap) b = kCap - 1;
+            bk[i] = b;
+            slot[i] = atomicAdd(&sm.cnt[b], 1u);
+        }
+    }
+    __syncthreads();
+    // exclusive scan of the kCap counters (kMItems consecutive counters per thread)
+    {
+        uint32_t c[kMItems], s = 0;
+#pragma unroll
+        for (int i = 0; i < kMItems; ++i) { c[i] = sm.cnt[tid * kMItems + i]; s += c[i]; }
+        uint32_t total;
+        uint32_t ex = block_exclusive_scan(s, sm.scan, &total);
+#pragma unroll
+        for (int i = 0; i < kMItems; ++i) { sm.cnt[tid * kMItems + i] = ex; ex += c[i]; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kMItems; ++i) {
+        const uint32_t e = tid + i * kMThreads;
+        if (e < count) sm.list[sm.cnt[bk[i]] + slot[i]] = (uint16_t)e;
+    }
+    __syncthreads();
+    // exact rank inside the bucket: order by (key, element id) = (time, input order)
+#pragma unroll
+    for (int i = 0; i < kMItems; ++i) {
+        const uint32_t e = tid + i * kMThreads;
+        if (e < count) {
+            const uint64_t key = key_of(hit_time(sm.tile[e]));
+            const uint32_t s0 = sm.cnt[bk[i]];
+            const uint32_t s1 = bk[i] + 1 < (uint32_t)kCap ? sm.cnt[bk[i] + 1] : count;
+            uint32_t r = s0;
+            for (uint32_t m = s0; m < s1; ++m) {
+                const uint32_t o = sm.list[m];
+                if (o != e) {
+                    const uint64_t ko = key_of(hit_time(sm.tile[o]));
+                    r += (ko < key || (ko == key && o < e)) ? 1u : 0u;
+                }
+            }
+            sm.inv[r] = (uint16_t)e;
+        }
+    }
+    __syncthreads();
+    // coalesced output
+    for (uint32_t r = tid; r < count; r += kMThreads) {
+        const uint32_t e = sm.inv[r];
+        out[out_base + r] = sm.tile[e];
+        if (kPerm) {
+            uint32_t lo = 0, hi = K;  // piece j with segstart[j] <= e < segstart[j+1]
+            while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.segstart[mid] <= e) lo = mid; else hi = mid; }
+            const uint32_t src = sm.cur[lo] + (e - sm.segstart[lo]);
+            perm_out[out_base + r] = perm_in ? perm_in[src] : src;
+        }
+    }
+    __syncthreads();
+    return count;
+}
+
+template <bool kPerm>
+__global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, const uint4* __restrict__ in,
+                                                                  uint4* __restrict__ out,
+                                                                  const uint32_t* __restrict__ perm_in,
+                                                                  uint32_t* __restrict__ perm_out, int check_runs,
+                                                                  int32_t* __restrict__ status) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    MergeSmem& sm = *reinterpret_cast<MergeSmem*>(smem_raw);
+    const uint32_t tid = threadIdx.x;
+    // which (group, tile)?
+    uint32_t lo = 0, hi = lv.G;
+    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (lv.tbase[mid] <= blockIdx.x) lo = mid; else hi = mid; }
+    const uint32_t g = lo, k = blockIdx.x - lv.tbase[g];
+    const uint32_t r0 = lv.gfirst[g], K = lv.gfirst[g + 1] - r0;
+    const uint32_t nt = lv.tbase[g + 1] - lv.tbase[g];
+    const uint32_t* row0 = lv.splits + lv.sbase[g] + (size_t)k * K;
+    const uint32_t* row1 = row0 + K;
+    const uint32_t* run_begin = lv.roff + r0;
+    uint32_t before = 0, len = 0;
+    if (tid < K) {
+        const uint32_t a = row0[tid];
+        uint32_t b = row1[tid];
+        if (b < a) b = a;  // only with unsorted runs (flagged by the run check)
+        sm.cur[tid] = a;
+        sm.end[tid] = b;
+        before = a - run_begin[tid];
+        len = b - a;
+    }
+    uint32_t out_base = lv.roff[r0] + block_sum(before, sm.scan);
+    uint32_t remaining = block_sum(len, sm.scan);
+    __syncthreads();
+    const uint64_t T0 = lv.gT0[g], DT = lv.gDT[g];
+    uint64_t Ta = T0 + (uint64_t)k * DT;
+    if (Ta < T0) Ta = ~0ull;
+    (void)nt;
+    if (remaining <= (uint32_t)kCap) {  // the common case: the whole tile in one chunk
+        if (remaining)
+            sort_chunk<kPerm>(sm, in, out, K, sm.end, Ta, DT, out_base, perm_in, perm_out, check_runs != 0, run_begin, status);
+        return;
+    }
+    // ---- overflow sweep: chunks of <= kCap hits in key order ------------------------------------------
+    while (remaining) {
+        // key range of what is left
+        uint64_t kmin = ~0ull, kmax = 0;
+        if (tid < K && sm.end[tid] > sm.cur[tid]) { kmin = key_at(in, sm.cur[tid]); kmax = key_at(in, sm.end[tid] - 1); }
+#pragma unroll
+        for (int d = 16; d; d >>= 1) {
+            const uint64_t o0 = __shfl_xor_sync(0xffffffffu, kmin, d), o1 = __shfl_xor_sync(0xffffffffu, kmax, d);
+            kmin = o0 < kmin ? o0 : kmin;
+            kmax = o1 > kmax ? o1 : kmax;
+        }
+        if ((tid & 31) == 0) { sm.red64[2 * (tid >> 5)] = kmin; sm.red64[2 * (tid >> 5) + 1] = kmax; }
+        __syncthreads();
+        kmin = ~0ull; kmax = 0;
+        for (int w = 0; w < kMThreads / 32; ++w) {
+            kmin = sm.red64[2 * w] < kmin ? sm.red64[2 * w] : kmin;
+            kmax = sm.red64[2 * w + 1] > kmax ? sm.red64[2 * w + 1] : kmax;
+        }
+        __syncthreads();
+        if (remaining <= (uint32_t)kCap) {
+            const uint32_t c = sort_chunk<kPerm>(sm, in, out, K, sm.end, kmin, kmax - kmin + 1 ? kmax - kmin + 1 : ~0ull,
+                                                 out_base, perm_in, perm_out, check_runs != 0, run_begin, status);
+            out_base += c;
+            break;
+        }
+        // largest x in [kmin, kmax) with C(x) = #{key <= x} <= kCap; C(kmax) = remaining > kCap.
+        // have_lo == false stands for x = kmin - 1 (C = 0).
+        bool have_lo = false;
+        uint64_t xlo = kmin, xhi = kmax;  // invariant: C(xlo) <= kCap (if have_lo) < C(xhi)
+        while (true) {
+            uint64_t xm;
+            if (!have_lo) {
+                if (xhi == kmin) break;  // even the single smallest key overflows: tie block
+                xm = kmin + ((xhi - kmin) >> 1);
+            } else {
+                if (xhi - xlo <= 1) break;
+                xm = xlo + ((xhi - xlo) >> 1);
+            }
+            uint32_t c = 0;
+            if (tid < K) {
+                uint32_t a = sm.cur[tid], b = sm.end[tid];
+                while (a < b) { const uint32_t mid = a + ((b - a) >> 1); if (key_at(in, mid) <= xm) a = mid + 1; else b = mid; }
+                sm.mid[tid] = a;
+                c = a - sm.cur[tid];
+            }
+            const uint32_t C = block_sum(c, sm.scan);
+            if (C <= (uint32_t)kCap) { have_lo = true; xlo = xm; } else xhi = xm;
+        }
+        // chunk end per run: keys <= xlo (or the tie block keys == kmin)
+        const uint64_t xcut = have_lo ? xlo : kmin;
+        uint32_t c = 0;
+        if (tid < K) {
+            uint32_t a = sm.cur[tid], b = sm.end[tid];
+            while (a < b) { const uint32_t mid = a + ((b - a) >> 1); if (key_at(in, mid) <= xcut) a = mid + 1; else b = mid; }
+            sm.mid[tid] = a;
+            c = a - sm.cur[tid];
+        }
+        uint32_t total;
+        const uint32_t ex = block_exclusive_scan(c, sm.scan, &total);
+        if (have_lo && total) {
+            sort_chunk<kPerm>(sm, in, out, K, sm.mid, kmin, xlo - kmin + 1, out_base, perm_in, perm_out, check_runs != 0,
+                              run_begin, status);
+        } else {
+            // tie block: every hit has key == kmin; the stable order is the run-major concatenation
+            if (tid < K) sm.segstart[tid] = ex;
+            if (tid == 0) sm.segstart[K] = total;
+            __syncthreads();
+            for (uint32_t e = tid; e < total; e += kMThreads) {
+                uint32_t lo2 = 0, hi2 = K;
+                while (hi2 - lo2 > 1) { const uint32_t mid = (lo2 + hi2) >> 1; if (sm.segstart[mid] <= e) lo2 = mid; else hi2 = mid; }
+                const uint32_t src = sm.cur[lo2] + (e - sm.segstart[lo2]);
+                out[out_base + e] = __ldg(in + src);
+                if (kPerm) perm_out[out_base + e] = perm_in ? perm_in[src] : src;
+            }
+            __syncthreads();
+        }
+        if (tid < K) sm.cur[tid] = sm.mid[tid];
+        out_base += total;
+        remaining -= total;
+        __syncthreads();
+    }
+}
+
+// ---- host side: plan mirror -----------------------------------------------------------------------------
+struct LevelHost {
+    std::vector<uint32_t> roff;  // run offsets of this level
+    uint32_t R, G, F, tiles, split_entries;
+    std::vector<uint32_t> next;  // group boundaries
+};
+
+static uint32_t lower_bound_u32(const std::vector<uint32_t>& v, uint32_t R, uint32_t x) {
+    uint32_t lo = 0, hi = R;
+    while (lo < hi) { const uint32_t mid = (lo + hi) >> 1; if (v[mid] < x) lo = mid + 1; else hi = mid; }
+    return lo;
+}
+
+static void plan_level(LevelHost& L, const uint32_t* h_seg, uint32_t n_seg, uint32_t n) {
+    L.tiles = 0; L.split_entries = 0; L.G = 0;
+    L.next.clear();
+    for (uint32_t s = 0; s < n_seg; ++s) {
+        const uint32_t r0 = lower_bound_u32(L.roff, L.R, h_seg[s]);
+        const uint32_t r1 = s + 1 == n_seg ? L.R : lower_bound_u32(L.roff, L.R, h_seg[s + 1]);
+        for (uint32_t r = r0; r < r1; r += L.F) {
+            const uint32_t re = r + L.F < r1 ? r + L.F : r1;
+            const uint32_t nt = tiles_for(L.roff[re] - L.roff[r]);
+            L.tiles += nt;
+            L.split_entries += nt ? (nt + 1) * (re - r) : 0;
+            L.next.push_back(L.roff[r]);
+            ++L.G;
+        }
+    }
+    L.next.push_back(n);
+}
+
+static void build_plan(std::vector<LevelHost>& levels, uint32_t n, const uint32_t* h_seg, uint32_t n_seg,
+                       const uint32_t* h_runs, uint32_t n_runs) {
+    // largest number of runs in one segment decides the number of levels and the fan-in
+    std::vector<uint32_t> roff(h_runs, h_runs + n_runs + 1);
+    uint32_t pmax = 1;
+    for (uint32_t s = 0; s < n_seg; ++s) {
+        const uint32_t r0 = lower_bound_u32(roff, n_runs, h_seg[s]);
+        const uint32_t r1 = s + 1 == n_seg ? n_runs : lower_bound_u32(roff, n_runs, h_seg[s + 1]);
+        if (r1 - r0 > pmax) pmax = r1 - r0;
+    }
+    uint32_t nlev = 1;
+    for (uint64_t cap = kMaxFan; cap < pmax; cap *= kMaxFan) ++nlev;
+    uint32_t F = kMaxFan;
+    if (nlev > 1) {  // smallest F with F^nlev >= pmax
+        F = 2;
+        while (true) {
+            uint64_t c = 1;
+            for (uint32_t l = 0; l < nlev; ++l) c *= F;
+            if (c >= pmax) break;
+            ++F;
+        }
+    }
+    levels.clear();
+    LevelHost L;
+    L.roff = roff; L.R = n_runs; L.F = F;
+    for (uint32_t l = 0; l < nlev; ++l) {
+        plan_level(L, h_seg, n_seg, n);
+        levels.push_back(L);
+        LevelHost N;
+        N.roff = L.next; N.R = L.G; N.F = F;
+        L = N;
+    }
+}
+
+struct MergeWs {
+    std::vector<LevelDev> dev;
+    uint4* tmp[2];
+    uint32_t* ptmp[2];
+};
+
+static void carve(Arena& a, const std::vector<LevelHost>& levels, uint32_t n, bool perm, MergeWs& w) {
+    w.dev.resize(levels.size());
+    for (size_t l = 0; l < levels.size(); ++l) {
+        const LevelHost& L = levels[l];
+        LevelDev& d = w.dev[l];
+        d.R = L.R; d.G = L.G; d.F = L.F;
+        d.gfirst = a.take<uint32_t>(L.G + 1);
+        d.tbase = a.take<uint32_t>(L.G + 1);
+        d.sbase = a.take<uint32_t>(L.G + 1);
+        d.gT0 = a.take<uint64_t>(L.G + 1);
+        d.gDT = a.take<uint64_t>(L.G + 1);
+        d.splits = a.take<uint32_t>((size_t)L.split_entries + 1);
+        d.roff_next = a.take<uint32_t>(L.G + 1);
+    }
+    const size_t nlev = levels.size();
+    w.tmp[0] = nlev > 1 ? a.take<uint4>(n) : nullptr;
+    w.tmp[1] = nlev > 2 ? a.take<uint4>(n) : nullptr;
+    w.ptmp[0] = (perm && nlev > 1) ? a.take<uint32_t>(n) : nullptr;
+    w.ptmp[1] = (perm && nlev > 2) ? a.take<uint32_t>(n) : nullptr;
+}
+
+size_t merge_ws_bytes(uint32_t n, const uint32_t* h_seg, uint32_t n_seg, const uint32_t* h_runs, uint32_t n_runs) {
+    std::vector<LevelHost> levels;
+    build_plan(levels, n, h_seg, n_seg, h_runs, n_runs);
+    Arena a(nullptr);
+    MergeWs w;
+    carve(a, levels, n, true, w);
+    return a.off;
+}
 
 int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, const uint32_t* d_seg_offsets,
-                    const uint32_t*, uint32_t n_seg, const uint32_t* d_run_offsets, const uint32_t*, uint32_t n_runs,
-                    void* d_ws, int32_t* d_status, cudaStream_t s) {
-    prof_mark(s, "sort.run_check");
-    TT_K(run_check_kernel)<<<div_up(n, 256), 256, 0, s>>>((const uint4*)d_in, n, d_run_offsets, n_runs, d_status);
-    return radix_sort(d_in, d_out, d_perm, n, d_seg_offsets, n_seg, d_ws, s);
+                    const uint32_t* h_seg, uint32_t n_seg, const uint32_t* d_run_offsets, const uint32_t* h_runs,
+                    uint32_t n_runs, void* d_ws, int32_t* d_status, cudaStream_t s) {
+    std::vector<LevelHost> levels;
+    build_plan(levels, n, h_seg, n_seg, h_runs, n_runs);
+    Arena a(d_ws);
+    MergeWs w;
+    carve(a, levels, n, true, w);
+    static bool attr_done = false;
+    if (!attr_done) {
+        TT_CUDA_OK(cudaFuncSetAttribute(merge_tile_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MergeSmem)));
+        TT_CUDA_OK(cudaFuncSetAttribute(merge_tile_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MergeSmem)));
+        attr_done = true;
+    }
+    const size_t nlev = levels.size();
+    const uint4* src = (const uint4*)d_in;
+    const uint32_t* psrc = nullptr;
+    for (size_t l = 0; l < nlev; ++l) {
+        LevelDev& d = w.dev[l];
+        d.roff = l == 0 ? d_run_offsets : w.dev[l - 1].roff_next;
+        const bool last = l + 1 == nlev;
+        uint4* dst = last ? (uint4*)d_out : w.tmp[l & 1];
+        uint32_t* pdst = d_perm ? (last ? d_perm : w.ptmp[l & 1]) : nullptr;
+        prof_mark(s, l == 0 ? "sort.merge_plan0" : "sort.merge_plan1");
+        TT_K(merge_groups_kernel)<<<1, 1024, 0, s>>>(d, d_seg_offsets, n_seg);
+        TT_K(merge_setup_kernel)<<<1, 1024, 0, s>>>(d, src, n);
+        if (levels[l].split_entries) {
+            prof_mark(s, l == 0 ? "sort.merge_partition0" : "sort.merge_partition1");
+            TT_K(merge_partition_kernel)<<<div_up(levels[l].split_entries, 256), 256, 0, s>>>(d, src, levels[l].split_entries);
+        }
+        if (levels[l].tiles) {
+            prof_mark(s, l == 0 ? "sort.merge_tile0" : "sort.merge_tile1");
+            if (d_perm)
+                TT_K(merge_tile_kernel<true>)<<<levels[l].tiles, kMThreads, sizeof(MergeSmem), s>>>(d, src, dst, psrc, pdst, l == 0, d_status);
+            else
+                TT_K(merge_tile_kernel<false>)<<<levels[l].tiles, kMThreads, sizeof(MergeSmem), s>>>(d, src, dst, nullptr, nullptr, l == 0, d_status);
+        }
+        src = dst;
+        psrc = pdst;
+    }
+    prof_end(s);
+    TT_LAUNCH_OK();
+    return TT_OK;
 }
+
 }  // namespace tt

@@ -206,3 +206,77 @@ def test_host_api_matches_device_api(B, oracle_lib):
     assert cnt[0] == len(o["seeds"]) and (seeds[: cnt[0]] == o["seeds"]).all()
     assert cnt[1] == len(o["events"]) and ev[: cnt[1]].tobytes() == o["events"].tobytes()
     L.tt_host_ctx_destroy(ctx)
+
+
+def _sort_only(B, h, seg, runs):
+    d_in = B.hits_to_device(h)
+    d_out = torch.empty_like(d_in)
+    d_perm = torch.empty(max(len(h), 1), dtype=torch.int32, device="cuda")
+    st = torch.zeros(1, dtype=torch.int32, device="cuda")
+    B.tt_sort_slice(d_in, d_out, d_perm, B.Offsets(seg), B.Offsets(runs) if runs is not None else None, st)
+    torch.cuda.synchronize()
+    return B.hits_to_host(d_out), d_perm.cpu().numpy().view(np.uint32)[: len(h)], int(st.item())
+
+
+def _as_runs(h, seg, n_pmt):
+    """Reorder arbitrary hits into PMT-major, time-ordered runs per segment; returns (hits, run offsets)."""
+    parts, offs = [], [0]
+    for a, b in zip(seg[:-1], seg[1:]):
+        sub = h[a:b]
+        o = np.lexsort((np.arange(len(sub)), sub["t_ps"], sub["pmt_id"]))
+        sub = sub[o]
+        parts.append(sub)
+        cnt = np.bincount(sub["pmt_id"], minlength=n_pmt)
+        for c in cnt:
+            offs.append(offs[-1] + int(c))
+    return np.concatenate(parts) if parts else h[:0], np.asarray(offs, dtype=np.uint32)
+
+
+@pytest.mark.parametrize("kind", ["tie_blocks", "skewed_density", "one_outlier", "three_levels", "many_empty_runs"])
+def test_merge_path_edge_cases(kind, B, oracle_lib):
+    """The run-merge path off its fast path: tiles that overflow the staging capacity (swept in
+    chunks), single timestamps with more hits than a chunk (tie blocks), a timestamp outlier that
+    stretches the key range, three merge levels, empty runs."""
+    rng = np.random.default_rng(21)
+    n_pmt = 84
+    if kind == "tie_blocks":
+        n = 60_000
+        h = np.zeros(n, dtype=W.HIT_DTYPE)
+        h["t_ps"] = rng.integers(0, 3, size=n)  # ~20 000 hits per timestamp >> 4096
+        seg = np.array([0, 25_000, n], dtype=np.uint32)
+    elif kind == "skewed_density":
+        n = 80_000
+        h = np.zeros(n, dtype=W.HIT_DTYPE)
+        t = rng.integers(0, 10**9, size=n)
+        t[: n // 2] = rng.integers(5 * 10**8, 5 * 10**8 + 10**6, size=n // 2)  # half of the hits in 0.1 % of the range
+        h["t_ps"] = t
+        seg = np.array([0, n], dtype=np.uint32)
+    elif kind == "one_outlier":
+        n = 40_000
+        h = np.zeros(n, dtype=W.HIT_DTYPE)
+        h["t_ps"] = rng.integers(0, 10**8, size=n)
+        h["t_ps"][7] = 2**62
+        h["t_ps"][9] = -2**62
+        seg = np.array([0, n], dtype=np.uint32)
+    elif kind == "three_levels":
+        n = 300_000  # every hit its own run: 300 000 > 512^2 runs -> three merge levels
+        h = np.zeros(n, dtype=W.HIT_DTYPE)
+        h["t_ps"] = rng.integers(0, 10**10, size=n)
+        seg = np.array([0, 100_000, n], dtype=np.uint32)
+    else:
+        n = 30_000
+        n_pmt = 3000  # most runs empty
+        h = np.zeros(n, dtype=W.HIT_DTYPE)
+        h["t_ps"] = rng.integers(0, 10**9, size=n)
+        seg = np.array([0, 0, 10_000, n, n], dtype=np.uint32)
+    h["pmt_id"] = rng.integers(0, n_pmt, size=n) if kind != "many_empty_runs" else rng.choice(np.arange(0, n_pmt, 7), size=n)
+    h["pad"] = np.arange(n) & 0xFFFF
+    if kind == "three_levels":
+        hr, runs = h, np.arange(n + 1, dtype=np.uint32)
+    else:
+        hr, runs = _as_runs(h, seg, n_pmt)
+    srt, perm = oracle.sort(hr, seg)
+    out, gperm, st = _sort_only(B, hr, seg, runs)
+    assert st == 0
+    assert out.tobytes() == srt.tobytes()
+    assert (gperm == perm).all()
