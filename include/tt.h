@@ -72,11 +72,13 @@ enum {
     TT_S_EVENT_OVERFLOW = 2, /* likewise for events                                                   */
     TT_S_RUN_UNSORTED = 4,   /* a run given by d_run_offsets is not non-decreasing: output unspecified */
     TT_S_BAD_PMT = 8,        /* an L1 hit has pmt_id >= n_pmt (it has no L2 edges)                     */
-    TT_S_DENSITY = 16        /* an L1 hit has more than TT_MAX_NEIGHBOURS causal neighbours: its L2STAR
-                                bit is exact, its clique-mode L2 bit is not decided (left clear)       */
+    TT_S_DENSITY = 16        /* an L1 hit has more than TT_MAX_NEIGHBOURS L1 hits of its segment within
+                                +-min(W, largest table entry) of it: its L2STAR bit is exact, its
+                                clique-mode L2 bit is not decided (left clear unless another hit's
+                                clique contains it)                                                  */
 };
 #define TT_MAX_MULTIPLICITY 16
-#define TT_MAX_NEIGHBOURS 256
+#define TT_MAX_NEIGHBOURS 2048
 
 /* Causality table dtmax[pmt_a][pmt_b] in integer ps (BASELINE.json configs[0]: d_ij*n/c + 20 ns,
  * precomputed by the caller), block-sparse by tower pair:

@@ -18,8 +18,9 @@ constexpr int kL1Threads = 256;
 struct L1Rec {  // compact L1 hit, 16 bytes
     int64_t t;
     uint32_t idx;  // index in the sorted hit array
-    uint32_t pmt;
+    uint32_t tp;   // tower << 16 | pmt index inside the tower; 0xFFFFFFFF = pmt_id out of range
 };
+constexpr uint32_t kBadTp = 0xFFFFFFFFu;
 
 __global__ void __launch_bounds__(kL1Threads) l1_flags_kernel(const uint4* __restrict__ hits, uint32_t n,
                                                               const uint32_t* __restrict__ seg_off, uint32_t n_seg,
@@ -61,125 +62,264 @@ __global__ void __launch_bounds__(kL1Threads) l1_flags_kernel(const uint4* __res
 __global__ void __launch_bounds__(kL1Threads) l1_compact_kernel(const uint4* __restrict__ hits, uint32_t n,
                                                                 const uint8_t* __restrict__ flags,
                                                                 const uint32_t* __restrict__ blk_off,
-                                                                L1Rec* __restrict__ l1) {
+                                                                L1Rec* __restrict__ l1, uint32_t n_pmt, uint32_t ppt,
+                                                                int32_t* __restrict__ status) {
     __shared__ uint32_t sm[33];
     const uint32_t i = blockIdx.x * kL1Threads + threadIdx.x;
     const bool is = i < n && (flags[i] & TT_L1);
     uint32_t total;
     const uint32_t r = block_exclusive_scan(is ? 1u : 0u, sm, &total);
+    bool bad = false;
     if (is) {
         const HitView h = unpack(__ldg(hits + i));
         L1Rec rec;
         rec.t = h.t;
         rec.idx = i;
-        rec.pmt = h.pmt;
+        if (h.pmt >= n_pmt) { rec.tp = kBadTp; bad = true; }
+        else { const uint32_t tw = h.pmt / ppt; rec.tp = (tw << 16) | (h.pmt - tw * ppt); }
         l1[blk_off[blockIdx.x] + r] = rec;
     }
+    if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(status, TT_S_BAD_PMT);
 }
 
 // ------------------------------------------------------------------------------------------------
-// L2: one warp per L1 hit.
+// L2.  Causality edge between two L1 hits; tp = tower << 16 | local pmt.
 // ------------------------------------------------------------------------------------------------
-constexpr int kL2Warps = 4;
-constexpr int kMaxNb = TT_MAX_NEIGHBOURS;  // 256
-constexpr int kMaxWords = kMaxNb / 32;     // 8
-
-struct L2Smem {
-    int64_t nb_t[kMaxNb];
-    uint32_t nb_p[kMaxNb];
-    uint32_t adj[kMaxNb * kMaxWords];
-};
-
-// dtmax lookup; -1 = never an edge.  a, b < n_pmt.
-__device__ __forceinline__ int32_t dtmax_of(const tt_geometry_dev& g, uint32_t a, uint32_t b) {
-    uint32_t ra = a, rb = b, blk = 0;
+__device__ __forceinline__ bool edge_tp(const tt_geometry_dev& g, uint64_t W, uint64_t dt, uint32_t tpa, uint32_t tpb) {
+    if (tpa == kBadTp || tpb == kBadTp) return false;
+    uint32_t blk = 0;
     if (g.n_tower > 1) {
-        const uint32_t ta = a / g.ppt, tb = b / g.ppt;
-        const int32_t bi = __ldg(g.pair_block + ta * g.n_tower + tb);
-        if (bi < 0) return -1;
+        const int32_t bi = __ldg(g.pair_block + (tpa >> 16) * g.n_tower + (tpb >> 16));
+        if (bi < 0) return false;
         blk = (uint32_t)bi;
-        ra = a - ta * g.ppt;
-        rb = b - tb * g.ppt;
     } else {
         const int32_t bi = __ldg(g.pair_block);
-        if (bi < 0) return -1;
+        if (bi < 0) return false;
         blk = (uint32_t)bi;
     }
-    return __ldg(g.blocks + ((size_t)blk * g.ppt + ra) * g.ppt + rb);
-}
-
-__device__ __forceinline__ bool edge_of(const tt_geometry_dev& g, uint64_t W, int64_t ta, uint32_t pa, int64_t tb,
-                                        uint32_t pb) {
-    if (pa >= g.n_pmt || pb >= g.n_pmt) return false;
-    const int32_t lim = dtmax_of(g, pa, pb);
+    const int32_t lim = __ldg(g.blocks + ((size_t)blk * g.ppt + (tpa & 0xFFFFu)) * g.ppt + (tpb & 0xFFFFu));
     if (lim < 0) return false;
-    const uint64_t d = ta >= tb ? udiff(ta, tb) : udiff(tb, ta);
     const uint64_t l = (uint64_t)lim < W ? (uint64_t)lim : W;
-    return d <= l;
+    return dt <= l;
+}
+__device__ __forceinline__ uint64_t absdiff(int64_t a, int64_t b) { return a >= b ? udiff(a, b) : udiff(b, a); }
+
+// ---- fast path, pass 1: neighbour rows.  One thread per L1 hit x; the candidates (L1 hits of the same
+// segment within +-Weff) are staged in shared memory per tile of 256 hits.  Row of x: lo = index of
+// the first candidate, 128-bit mask of the causal neighbours relative to lo.  A hit with more than
+// 128 candidates ("wide") goes to the slow list instead.
+constexpr int kRowTile = 256;
+constexpr int kRowStage = 1536;   // staged records per tile (tile + halos)
+constexpr uint32_t kWide = 0xFFFFFFFFu;
+
+struct Row {  // 32 bytes
+    uint64_t m0, m1;
+    uint32_t lo, deg;
+    uint32_t pad0, pad1;
+};
+
+__global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restrict__ l1, const uint32_t* __restrict__ m_ptr,
+                                                           const uint32_t* __restrict__ seg_off, uint32_t n_seg,
+                                                           uint32_t n, tt_geometry_dev g, uint64_t W, uint32_t N,
+                                                           uint32_t mode, uint8_t* __restrict__ flags,
+                                                           uint8_t* __restrict__ l2bit, Row* __restrict__ rows,
+                                                           uint32_t* __restrict__ slow_list, uint32_t* __restrict__ slow_cnt) {
+    __shared__ int64_t s_t[kRowStage];
+    __shared__ uint32_t s_idx[kRowStage];
+    __shared__ uint32_t s_tp[kRowStage];
+    __shared__ uint32_t s_range[2];
+    const uint32_t m = *m_ptr;
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const bool any_edge = g.max_dt >= 0;
+    const uint64_t Weff = any_edge ? ((uint64_t)g.max_dt < W ? (uint64_t)g.max_dt : W) : 0;
+    const uint32_t ntiles = (m + kRowTile - 1) / kRowTile;
+    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const uint32_t x0 = tile * kRowTile, x1 = min(m, x0 + kRowTile);
+        // stage range: [lo(x0), hi(x1-1)) -- warp 0 scans backwards from x0, warp 1 forwards from x1-1
+        if (warp == 0) {
+            const L1Rec r0 = l1[x0];
+            uint32_t sa = 0;
+            if (n_seg > 1) sa = __ldg(seg_off + find_segment(seg_off, n_seg, r0.idx));
+            uint32_t lo = x0;
+            for (uint32_t base = x0; base > 0;) {
+                const bool valid = base > lane;
+                bool in = false;
+                if (valid) { const L1Rec ry = l1[base - 1 - lane]; in = ry.idx >= sa && udiff(r0.t, ry.t) <= Weff; }
+                const uint32_t ib = __ballot_sync(0xffffffffu, in);
+                lo = base - __popc(ib);  // `in` is monotone: a prefix of the lanes
+                if (ib != 0xffffffffu) break;
+                base -= 32;
+            }
+            if (lane == 0) s_range[0] = lo;
+        } else if (warp == 1) {
+            const L1Rec r1 = l1[x1 - 1];
+            uint32_t sb = n;
+            if (n_seg > 1) sb = __ldg(seg_off + find_segment(seg_off, n_seg, r1.idx) + 1);
+            uint32_t hi = x1;
+            for (uint32_t base = x1; base < m; base += 32) {
+                const uint32_t y = base + lane;
+                bool in = false;
+                if (y < m) { const L1Rec ry = l1[y]; in = ry.idx < sb && udiff(ry.t, r1.t) <= Weff; }
+                const uint32_t ib = __ballot_sync(0xffffffffu, in);
+                hi = base + __popc(ib);
+                if (ib != 0xffffffffu) break;
+            }
+            if (lane == 0) s_range[1] = hi;
+        }
+        __syncthreads();
+        const uint32_t ylo = s_range[0], yhi = s_range[1];
+        const bool staged = yhi - ylo <= (uint32_t)kRowStage;
+        if (staged)
+            for (uint32_t y = ylo + tid; y < yhi; y += kRowTile) {
+                const L1Rec r = l1[y];
+                s_t[y - ylo] = r.t; s_idx[y - ylo] = r.idx; s_tp[y - ylo] = r.tp;
+            }
+        __syncthreads();
+        const uint32_t x = x0 + tid;
+        if (x < x1) {
+            bool wide = !staged;
+            Row row;
+            row.m0 = row.m1 = 0; row.lo = kWide; row.deg = 0; row.pad0 = row.pad1 = 0;
+            if (staged) {
+                const uint32_t xl = x - ylo, cnt = yhi - ylo;
+                const int64_t tx = s_t[xl];
+                const uint32_t ix = s_idx[xl], tpx = s_tp[xl];
+                uint32_t sa = 0, sb = n;
+                if (n_seg > 1) {
+                    const uint32_t s = find_segment(seg_off, n_seg, ix);
+                    sa = __ldg(seg_off + s); sb = __ldg(seg_off + s + 1);
+                }
+                // first y <= x with idx >= sa and tx - t_y <= Weff (monotone false..true on [0, xl])
+                uint32_t a = 0, b = xl;
+                while (a < b) { const uint32_t mid = (a + b) >> 1; if (s_idx[mid] >= sa && udiff(tx, s_t[mid]) <= Weff) b = mid; else a = mid + 1; }
+                const uint32_t lo = a;
+                // first y > x that is out (idx >= sb or t_y - tx > Weff): monotone true..false on (xl, cnt)
+                a = xl + 1; b = cnt;
+                while (a < b) { const uint32_t mid = (a + b) >> 1; if (s_idx[mid] < sb && udiff(s_t[mid], tx) <= Weff) a = mid + 1; else b = mid; }
+                const uint32_t hi = a;
+                if (hi - lo > 128) wide = true;
+                else {
+                    uint64_t m0 = 0, m1 = 0;
+                    if (any_edge && tpx != kBadTp) {
+                        for (uint32_t y = lo; y < hi; ++y) {
+                            if (y == xl) continue;
+                            const bool e = edge_tp(g, W, absdiff(tx, s_t[y]), tpx, s_tp[y]);
+                            const uint32_t k = y - lo;
+                            if (e) { if (k < 64) m0 |= 1ull << k; else m1 |= 1ull << (k - 64); }
+                        }
+                    }
+                    row.m0 = m0; row.m1 = m1; row.lo = ylo + lo;
+                    row.deg = __popcll(m0) + __popcll(m1);
+                }
+            }
+            rows[x] = row;
+            if (wide) {
+                l2bit[x] = 0;
+                slow_list[atomicAdd(slow_cnt, 1u)] = x;
+            } else {
+                const bool star = row.deg + 1 >= N;
+                const bool decided = mode == 1 || N <= 2 || !star;  // clique test needed only for star hits, N > 2
+                uint32_t f = 0;
+                if (star) f |= TT_L2STAR;
+                if (decided && star) f |= TT_L2;
+                if (f) flags[l1[x].idx] |= (uint8_t)f;
+                l2bit[x] = (decided && star) ? 1 : 0;
+            }
+        }
+        __syncthreads();
+    }
 }
 
-// Is there a clique of `K` vertices in the graph (deg vertices, adjacency rows of `words` words)?
-// Each lane starts from its own smallest vertex; iterative DFS on candidate bitmasks.
-__device__ bool warp_has_clique(const uint32_t* adj, int deg, int words, int K, uint32_t lane) {
-    bool found = false;
-    if (K <= 0) found = true;
-    uint32_t cand[TT_MAX_MULTIPLICITY][kMaxWords];
-    for (int u = (int)lane; u < deg && !found; u += 32) {
-        if (K == 1) { found = true; break; }
-        const int need = K - 1;  // vertices still to choose after u
-        // cand[0] = adj[u] restricted to vertices > u
-        int cnt = 0;
-        for (int w = 0; w < words; ++w) {
-            uint32_t m = adj[u * words + w];
-            if (w < (u >> 5)) m = 0;
-            else if (w == (u >> 5)) m &= ~((2u << (u & 31)) - 1u);
-            cand[0][w] = m;
-            cnt += __popc(m);
-        }
-        (void)cnt;
+// ---- fast path, pass 2: exact clique test on the rows (no table lookups).  One thread per star hit.
+struct M128 { uint64_t a, b; };
+__device__ __forceinline__ M128 m_and(M128 x, M128 y) { return {x.a & y.a, x.b & y.b}; }
+__device__ __forceinline__ int m_pop(M128 x) { return __popcll(x.a) + __popcll(x.b); }
+__device__ __forceinline__ M128 m_shl(M128 x, uint32_t s) {  // s < 128
+    if (s == 0) return x;
+    if (s >= 64) return {0ull, x.a << (s - 64)};
+    return {x.a << s, (x.b << s) | (x.a >> (64 - s))};
+}
+__device__ __forceinline__ M128 m_shr(M128 x, uint32_t s) {
+    if (s == 0) return x;
+    if (s >= 64) return {x.b >> (s - 64), 0ull};
+    return {(x.a >> s) | (x.b << (64 - s)), x.b >> s};
+}
+
+__global__ void __launch_bounds__(128) l2_clique_kernel(const L1Rec* __restrict__ l1, const uint32_t* __restrict__ m_ptr,
+                                                        const Row* __restrict__ rows, uint32_t N, uint32_t mode,
+                                                        uint8_t* __restrict__ flags, uint8_t* __restrict__ l2bit,
+                                                        uint32_t* __restrict__ slow_list, uint32_t* __restrict__ slow_cnt) {
+    if (mode != 0 || N <= 2) return;
+    const uint32_t m = *m_ptr;
+    const int K = (int)N - 1;  // clique size wanted among the neighbours of x
+    for (uint32_t x = blockIdx.x * blockDim.x + threadIdx.x; x < m; x += gridDim.x * blockDim.x) {
+        const Row rx = rows[x];
+        if (rx.lo == kWide || rx.deg + 1 < N) continue;
+        const M128 nx = {rx.m0, rx.m1};
+        M128 cand[TT_MAX_MULTIPLICITY];
+        cand[0] = nx;
         int d = 0;
+        bool found = false, punt = false;
         while (true) {
-            const int rem = need - d;
+            const int rem = K - d;
             if (rem == 0) { found = true; break; }
-            int pc = 0;
-            for (int w = 0; w < words; ++w) pc += __popc(cand[d][w]);
-            if (pc < rem) {
+            if (m_pop(cand[d]) < rem) {
                 if (d == 0) break;
                 --d;
                 continue;
             }
-            // pick the lowest candidate v, remove it, descend with cand & adj[v]
-            int v = -1;
-            for (int w = 0; w < words; ++w) {
-                if (cand[d][w]) {
-                    const int bit = __ffs(cand[d][w]) - 1;
-                    cand[d][w] &= cand[d][w] - 1u;
-                    v = w * 32 + bit;
-                    break;
-                }
-            }
-            for (int w = 0; w < words; ++w) cand[d + 1][w] = cand[d][w] & adj[v * words + w];
+            // lowest candidate v (x frame), remove it, descend with cand & adj(v)
+            int v;
+            if (cand[d].a) { v = __ffsll((long long)cand[d].a) - 1; cand[d].a &= cand[d].a - 1; }
+            else { v = 64 + __ffsll((long long)cand[d].b) - 1; cand[d].b &= cand[d].b - 1; }
+            const Row rv = rows[rx.lo + (uint32_t)v];
+            if (rv.lo == kWide) { punt = true; break; }
+            M128 av = {rv.m0, rv.m1};
+            av = rv.lo >= rx.lo ? m_shl(av, rv.lo - rx.lo) : m_shr(av, rx.lo - rv.lo);  // |shift| < 128 (windows overlap)
+            cand[d + 1] = m_and(cand[d], av);
             ++d;
         }
+        if (punt) {
+            slow_list[atomicAdd(slow_cnt, 1u)] = x;
+        } else if (found) {
+            flags[l1[x].idx] |= (uint8_t)TT_L2;
+            l2bit[x] = 1;
+        }
     }
-    return __any_sync(0xffffffffu, found);
 }
 
-__global__ void __launch_bounds__(kL2Warps * 32) l2_kernel(const L1Rec* __restrict__ l1,
-                                                           const uint32_t* __restrict__ m_ptr,
-                                                           const uint32_t* __restrict__ seg_off, uint32_t n_seg,
-                                                           uint32_t n, tt_geometry_dev g, uint64_t W, uint32_t N,
-                                                           uint32_t mode, uint8_t* __restrict__ flags,
-                                                           uint8_t* __restrict__ l2bit, int32_t* __restrict__ status) {
+// ---- wide path: one warp per listed L1 hit (windows of more than 128 candidates: muon tracks, bursts).
+// The window [lo, hi) of x is a bitmask of up to kMaxWin candidates in shared memory; the clique search is
+// a lazy depth-first search: mask[d+1] = {c in mask[d] : edge(v, c)} is evaluated on demand for the picked
+// vertex v only, so a dense clique (a track) is found after N-2 refinements instead of a full adjacency
+// matrix.  A found clique marks ALL its members L2 (each of them is in an N-clique), which lets the other
+// hits of the same track skip their own search.
+constexpr int kL2Warps = 4;
+constexpr int kMaxWin = TT_MAX_NEIGHBOURS;   // candidates per window
+constexpr int kWinWords = kMaxWin / 32;
+
+struct WideSmem {
+    uint32_t mask[TT_MAX_MULTIPLICITY][kWinWords];
+};
+
+__global__ void __launch_bounds__(kL2Warps * 32) l2_wide_kernel(const L1Rec* __restrict__ l1,
+                                                                const uint32_t* __restrict__ m_ptr,
+                                                                const uint32_t* __restrict__ slow_list,
+                                                                const uint32_t* __restrict__ slow_cnt,
+                                                                const uint32_t* __restrict__ seg_off, uint32_t n_seg,
+                                                                uint32_t n, tt_geometry_dev g, uint64_t W, uint32_t N,
+                                                                uint32_t mode, uint8_t* flags, volatile uint8_t* l2bit,
+                                                                int32_t* __restrict__ status) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    L2Smem& sm = reinterpret_cast<L2Smem*>(smem_raw)[warp];
-    const uint32_t m = *m_ptr;
+    WideSmem& sm = reinterpret_cast<WideSmem*>(smem_raw)[warp];
+    const uint32_t m = *m_ptr, nlist = *slow_cnt;
     const uint32_t nwarps = gridDim.x * kL2Warps;
-    // effective scan window: no edge can be longer than the largest table entry
     const bool any_edge = g.max_dt >= 0;
     const uint64_t Weff = any_edge ? ((uint64_t)g.max_dt < W ? (uint64_t)g.max_dt : W) : 0;
-    for (uint32_t x = blockIdx.x * kL2Warps + warp; x < m; x += nwarps) {
+    const int K = (int)N - 1;
+    for (uint32_t q = blockIdx.x * kL2Warps + warp; q < nlist; q += nwarps) {
+        const uint32_t x = slow_list[q];
         const L1Rec rx = l1[x];
         uint32_t sa = 0, sb = n;
         if (n_seg > 1) {
@@ -187,82 +327,113 @@ __global__ void __launch_bounds__(kL2Warps * 32) l2_kernel(const L1Rec* __restri
             sa = __ldg(seg_off + s);
             sb = __ldg(seg_off + s + 1);
         }
-        const bool bad = rx.pmt >= g.n_pmt;
-        if (bad && lane == 0) atomicOr(status, TT_S_BAD_PMT);
-        uint32_t deg = 0;
-        if (!bad && any_edge) {
-            // backward
-            for (uint32_t base = x; base > 0;) {
-                const bool valid = base > lane;  // y = base-1-lane >= 0
-                const uint32_t y = valid ? base - 1 - lane : 0;
-                bool in = false, e = false;
-                L1Rec ry;
-                if (valid) {
-                    ry = l1[y];
-                    in = ry.idx >= sa && udiff(rx.t, ry.t) <= Weff;
-                    if (in) e = edge_of(g, W, rx.t, rx.pmt, ry.t, ry.pmt);
-                }
-                const uint32_t eb = __ballot_sync(0xffffffffu, e);
-                const uint32_t ib = __ballot_sync(0xffffffffu, in);
-                if (e) {
-                    const uint32_t pos = deg + __popc(eb & lanemask_lt());
-                    if (pos < (uint32_t)kMaxNb) { sm.nb_t[pos] = ry.t; sm.nb_p[pos] = ry.pmt; }
-                }
-                deg += __popc(eb);
-                if (ib != 0xffffffffu) break;
-                base -= 32;  // ib full => base > 31
-            }
-            // forward
-            for (uint32_t base = x + 1; base < m; base += 32) {
-                const uint32_t y = base + lane;
-                const bool valid = y < m;
-                bool in = false, e = false;
-                L1Rec ry;
-                if (valid) {
-                    ry = l1[y];
-                    in = ry.idx < sb && udiff(ry.t, rx.t) <= Weff;
-                    if (in) e = edge_of(g, W, rx.t, rx.pmt, ry.t, ry.pmt);
-                }
-                const uint32_t eb = __ballot_sync(0xffffffffu, e);
-                const uint32_t ib = __ballot_sync(0xffffffffu, in);
-                if (e) {
-                    const uint32_t pos = deg + __popc(eb & lanemask_lt());
-                    if (pos < (uint32_t)kMaxNb) { sm.nb_t[pos] = ry.t; sm.nb_p[pos] = ry.pmt; }
-                }
-                deg += __popc(eb);
-                if (ib != 0xffffffffu) break;
-            }
+        // window extents
+        uint32_t lo = x, hi = x + 1;
+        for (uint32_t base = x; base > 0;) {
+            const bool valid = base > lane;
+            bool in = false;
+            if (valid) { const L1Rec ry = l1[base - 1 - lane]; in = ry.idx >= sa && udiff(rx.t, ry.t) <= Weff; }
+            const uint32_t ib = __ballot_sync(0xffffffffu, in);
+            lo = base - __popc(ib);
+            if (ib != 0xffffffffu) break;
+            base -= 32;
         }
+        for (uint32_t base = x + 1; base < m; base += 32) {
+            const uint32_t y = base + lane;
+            bool in = false;
+            if (y < m) { const L1Rec ry = l1[y]; in = ry.idx < sb && udiff(ry.t, rx.t) <= Weff; }
+            const uint32_t ib = __ballot_sync(0xffffffffu, in);
+            hi = base + __popc(ib);
+            if (ib != 0xffffffffu) break;
+        }
+        const uint32_t w = hi - lo;
+        const bool fits = w <= (uint32_t)kMaxWin;
+        const uint32_t nwords = (w + 31) >> 5;
+        const bool live = rx.tp != kBadTp && any_edge;
+        // neighbours of x
+        uint32_t deg = 0;
+        for (uint32_t k = 0; k < nwords; ++k) {
+            const uint32_t y = lo + 32 * k + lane;
+            bool e = false;
+            if (live && y < hi && y != x) { const L1Rec ry = l1[y]; e = edge_tp(g, W, absdiff(rx.t, ry.t), rx.tp, ry.tp); }
+            const uint32_t eb = __ballot_sync(0xffffffffu, e);
+            if (fits && lane == 0) sm.mask[0][k] = eb;
+            deg += __popc(eb);
+        }
+        __syncwarp();
         const bool star = deg + 1 >= N;
         bool l2 = star;
         if (star && mode == 0 && N > 2) {
-            if (deg > (uint32_t)kMaxNb) {
-                l2 = false;
+            l2 = false;
+            if (!fits) {
                 if (lane == 0) atomicOr(status, TT_S_DENSITY);
+            } else if (l2bit[x]) {
+                l2 = true;  // already marked as a member of a clique found from another hit
             } else {
-                __syncwarp();
-                const int words = (int)((deg + 31) >> 5);
-                for (uint32_t u = 0; u < deg; ++u) {
-                    const int64_t tu = sm.nb_t[u];
-                    const uint32_t pu = sm.nb_p[u];
-                    for (int w = 0; w < words; ++w) {
-                        const uint32_t v = w * 32 + lane;
-                        const bool e = v < deg && v != u && edge_of(g, W, tu, pu, sm.nb_t[v], sm.nb_p[v]);
-                        const uint32_t eb = __ballot_sync(0xffffffffu, e);
-                        if (lane == 0) sm.adj[u * words + w] = eb;
+                // need K vertices of mask[0], pairwise adjacent
+                uint32_t cnt[TT_MAX_MULTIPLICITY];
+                uint32_t chosen[TT_MAX_MULTIPLICITY];
+                cnt[0] = deg;
+                int d = 0;
+                while (true) {
+                    const int rem = K - d;
+                    if (cnt[d] < (uint32_t)rem) {
+                        if (d == 0) break;
+                        --d;
+                        continue;
+                    }
+                    // lowest candidate v of mask[d]
+                    uint32_t v = 0xFFFFFFFFu;
+                    for (uint32_t k0 = 0; k0 < nwords; k0 += 32) {
+                        const uint32_t k = k0 + lane;
+                        const uint32_t wv = k < nwords ? sm.mask[d][k] : 0u;
+                        const uint32_t nz = __ballot_sync(0xffffffffu, wv != 0);
+                        if (nz) {
+                            const uint32_t src = __ffs(nz) - 1;
+                            const uint32_t word = __shfl_sync(0xffffffffu, wv, src);
+                            v = (k0 + src) * 32 + (__ffs(word) - 1);
+                            break;
+                        }
+                    }
+                    chosen[d] = v;
+                    if (rem == 1) { l2 = true; break; }
+                    if (lane == 0) sm.mask[d][v >> 5] &= ~(1u << (v & 31));
+                    cnt[d] -= 1;
+                    __syncwarp();
+                    const L1Rec rv = l1[lo + v];
+                    uint32_t c = 0;
+                    for (uint32_t k = 0; k < nwords; ++k) {
+                        uint32_t nw = 0;
+                        if (k >= (v >> 5)) {
+                            const uint32_t bits = sm.mask[d][k];
+                            bool e = false;
+                            if ((bits >> lane) & 1u) {
+                                const L1Rec ry = l1[lo + 32 * k + lane];
+                                e = edge_tp(g, W, absdiff(rv.t, ry.t), rv.tp, ry.tp);
+                            }
+                            nw = __ballot_sync(0xffffffffu, e);
+                        }
+                        if (lane == 0) sm.mask[d + 1][k] = nw;
+                        c += __popc(nw);
+                    }
+                    __syncwarp();
+                    cnt[d + 1] = c;
+                    ++d;
+                }
+                if (l2 && lane == 0) {  // mark the other members of the clique
+                    for (int q2 = 0; q2 < K; ++q2) {
+                        const uint32_t y = lo + chosen[q2];
+                        l2bit[y] = 1;  // its TT_L2 flag is set by seed_write_kernel
                     }
                 }
-                __syncwarp();
-                l2 = warp_has_clique(sm.adj, (int)deg, words, (int)N - 1, lane);
-                __syncwarp();
             }
         }
         if (lane == 0) {
             uint32_t f = 0;
             if (star) f |= TT_L2STAR;
             if (l2) f |= TT_L2;
-            if (f) flags[rx.idx] |= (uint8_t)f;
-            l2bit[x] = l2 ? 1 : 0;
+            if (f) flags[rx.idx] |= (uint8_t)f;  // only this warp touches this byte here
+            if (l2) l2bit[x] = 1;
         }
         __syncwarp();
     }
@@ -319,7 +490,8 @@ __global__ void __launch_bounds__(kSeedThreads) seed_write_kernel(const uint8_t*
                                                                   const L1Rec* __restrict__ l1,
                                                                   const uint32_t* __restrict__ m_ptr,
                                                                   const uint32_t* __restrict__ off,
-                                                                  uint32_t* __restrict__ seeds, uint32_t cap) {
+                                                                  uint32_t* __restrict__ seeds, uint32_t cap,
+                                                                  uint8_t* __restrict__ flags) {
     __shared__ uint32_t sm[33];
     uint32_t c0, c1;
     chunk_bounds(*m_ptr, c0, c1);
@@ -329,7 +501,11 @@ __global__ void __launch_bounds__(kSeedThreads) seed_write_kernel(const uint8_t*
         const bool is = x < c1 && l2bit[x];
         uint32_t total;
         const uint32_t r = block_exclusive_scan(is ? 1u : 0u, sm, &total);
-        if (is && run + r < cap) seeds[run + r] = l1[x].idx;
+        if (is) {
+            const uint32_t i = l1[x].idx;
+            flags[i] |= (uint8_t)TT_L2;  // idempotent; covers members marked by another hit's clique search
+            if (run + r < cap) seeds[run + r] = i;
+        }
         run += total;
     }
 }
@@ -339,6 +515,8 @@ struct TriggerPlan {
     uint32_t *blk_cnt, *scan_scratch, *m_total, *seed_cnt;
     L1Rec* l1;
     uint8_t* l2bit;
+    Row* rows;
+    uint32_t *slow_list, *slow_cnt;
     uint32_t nblk;
 };
 
@@ -350,6 +528,9 @@ static void trigger_plan(Arena& a, uint32_t n, TriggerPlan& p) {
     p.seed_cnt = a.take<uint32_t>(kSeedBlocks);
     p.l1 = a.take<L1Rec>(n);
     p.l2bit = a.take<uint8_t>(n);
+    p.rows = a.take<Row>(n);
+    p.slow_list = a.take<uint32_t>(n);
+    p.slow_cnt = a.take<uint32_t>(1);
 }
 
 }  // namespace tt
@@ -388,8 +569,8 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     trigger_plan(a, n, plan);
     static bool attr_done = false;
     if (!attr_done) {
-        TT_CUDA_OK(cudaFuncSetAttribute(l2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        (int)(sizeof(L2Smem) * kL2Warps)));
+        TT_CUDA_OK(cudaFuncSetAttribute(l2_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        (int)(sizeof(WideSmem) * kL2Warps)));
         attr_done = true;
     }
     prof_mark(s, "trig.l1_flags");
@@ -399,16 +580,25 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     int rc = exclusive_scan_u32(plan.blk_cnt, plan.blk_cnt, plan.nblk, plan.scan_scratch, plan.m_total, s);
     if (rc != TT_OK) return rc;
     prof_mark(s, "trig.l1_compact");
-    TT_K(l1_compact_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1);
-    prof_mark(s, "trig.l2");
-    TT_K(l2_kernel)<<<kSMs * 8, kL2Warps * 32, sizeof(L2Smem) * kL2Warps, s>>>(
-        plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps, p->l2_multiplicity,
-        p->l2_mode, d_flags, plan.l2bit, d_status);
+    TT_K(l1_compact_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1,
+                                                         g->dev.n_pmt, g->dev.ppt, d_status);
+    prof_mark(s, "trig.l2_rows");
+    TT_CUDA_OK(cudaMemsetAsync(plan.slow_cnt, 0, sizeof(uint32_t), s));
+    TT_K(l2_rows_kernel)<<<kSMs * 8, kRowTile, 0, s>>>(plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev,
+                                                      (uint64_t)p->l2_window_ps, p->l2_multiplicity, p->l2_mode, d_flags,
+                                                      plan.l2bit, plan.rows, plan.slow_list, plan.slow_cnt);
+    prof_mark(s, "trig.l2_clique");
+    TT_K(l2_clique_kernel)<<<kSMs * 16, 128, 0, s>>>(plan.l1, plan.m_total, plan.rows, p->l2_multiplicity, p->l2_mode,
+                                                     d_flags, plan.l2bit, plan.slow_list, plan.slow_cnt);
+    prof_mark(s, "trig.l2_wide");
+    TT_K(l2_wide_kernel)<<<kSMs * 4, kL2Warps * 32, sizeof(WideSmem) * kL2Warps, s>>>(
+        plan.l1, plan.m_total, plan.slow_list, plan.slow_cnt, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps,
+        p->l2_multiplicity, p->l2_mode, d_flags, plan.l2bit, d_status);
     prof_mark(s, "trig.seeds");
     TT_K(seed_count_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.m_total, plan.seed_cnt);
     TT_K(count_scan_kernel)<<<1, 1024, 0, s>>>(plan.seed_cnt, kSeedBlocks, d_n_seeds, seed_cap, TT_S_SEED_OVERFLOW, d_status);
     TT_K(seed_write_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.l1, plan.m_total, plan.seed_cnt, d_seeds,
-                                                           seed_cap);
+                                                           seed_cap, d_flags);
     prof_end(s);
     TT_LAUNCH_OK();
     return TT_OK;

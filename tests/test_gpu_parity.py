@@ -155,12 +155,12 @@ def test_status_codes(B, oracle_lib):
 
 
 def test_dense_neighbourhood(B, oracle_lib):
-    """A burst of mutually causal L1 hits: degrees far above 32 (multi-word masks), and above
-    TT_MAX_NEIGHBOURS (TT_S_DENSITY: star bit exact, clique bit left clear, status says so)."""
+    """Bursts of mutually causal L1 hits: windows above 128 candidates (wide path, lazy clique search) and
+    above TT_MAX_NEIGHBOURS = 2048 (TT_S_DENSITY: star bit exact, clique bit not decided, status says so)."""
     geo_w = W.make_geometry("km3")
     geo = _geo(B, geo_w)
     rng = np.random.default_rng(9)
-    for m, expect_density in ((150, False), (300, True)):
+    for m, expect_density in ((150, False), (700, False), (2500, True)):
         h = np.zeros(m + 200, dtype=W.HIT_DTYPE)
         h["pmt_id"] = rng.integers(0, 84, size=len(h))
         h["floor"] = geo_w.floor[h["pmt_id"]]
@@ -169,17 +169,35 @@ def test_dense_neighbourhood(B, oracle_lib):
         h["t_ps"][m:] = np.sort(rng.integers(2_000_000_000, 3_000_000_000, size=200))
         seg = np.array([0, len(h)], dtype=np.uint32)
         p = W.Params(l2_multiplicity=6)
-        o = oracle_chain(h, seg, geo_w, p)
+        if expect_density:
+            p_star = W.Params(l2_multiplicity=6, l2_mode=1)
+            o = oracle_chain(h, seg, geo_w, p_star)  # star bits only (the oracle's clique search is O(k^2) per hit)
+        else:
+            o = oracle_chain(h, seg, geo_w, p)
         r = B.process_slice(h, seg, None, geo, _prm(B, p))
         assert ((r.flags & 8) == (o["flags"] & 8)).all()
         if expect_density:
             assert r.status & B.TT_S_DENSITY
             dense = np.arange(len(h)) < m
-            assert ((r.flags & 16)[~dense] == (o["flags"] & 16)[~dense]).all()
             assert not (r.flags & 16)[dense].any()
         else:
             assert r.status == 0
             assert (r.flags == o["flags"]).all() and (r.seeds == o["seeds"]).all()
+    # a sparse graph on a wide window: many hits, few edges (table entries of 1 ps) -> search must exhaust
+    tab = np.full((84, 84), 1, dtype=np.int32)
+    tab[:6, :6] = 100_000
+    g2 = single_tower_geo(tab)
+    h = np.zeros(600, dtype=W.HIT_DTYPE)
+    h["pmt_id"] = rng.integers(0, 84, size=600)
+    h["charge"] = 500
+    h["t_ps"] = np.sort(rng.integers(0, 90_000, size=600))
+    seg = np.array([0, 600], dtype=np.uint32)
+    for N in (3, 4, 6):
+        p = W.Params(l2_multiplicity=N)
+        o = oracle_chain(h, seg, g2, p)
+        r = B.process_slice(h, seg, None, _geo(B, g2), _prm(B, p))
+        assert (r.flags == o["flags"]).all() and (r.seeds == o["seeds"]).all() and r.status == 0
+        assert 0 < len(o["seeds"]) < 600
 
 
 def test_host_api_matches_device_api(B, oracle_lib):
