@@ -38,6 +38,7 @@ struct LevelDev {
     uint64_t* gDT;           // [G] tile width in key units (>= 1)
     uint32_t* splits;        // split table
     uint32_t* roff_next;     // [G+1] run offsets of the next level (= group boundaries)
+    uint32_t* tile_g;        // [tiles] group of every tile
     uint32_t R, G, F;
 };
 
@@ -152,21 +153,51 @@ __global__ void __launch_bounds__(256) merge_partition_kernel(LevelDev lv, const
         res = a;
     }
     lv.splits[id] = res;
+    if (j == 0 && k < nt) lv.tile_g[lv.tbase[g] + k] = g;
 }
 
 // ---- the tile kernel ---------------------------------------------------------------------------------
 struct MergeSmem {
-    uint4 tile[kCap];             // staged records, run-major                       64 KB
-    uint32_t cnt[kCap];           // bucket counters -> exclusive starts             16 KB
-    uint16_t list[kCap];          // bucket member lists (tile-local element ids)     8 KB
-    uint16_t inv[kCap];           // inv[rank] = element id                           8 KB
+    uint4 tile[kCap];             // staged records, run-major (filled by TMA bulk copies)   64 KB
+    uint32_t cnt[kCap / 2];       // packed 16-bit bucket counters -> exclusive starts         8 KB
+    uint16_t list[kCap];          // bucket member lists (tile-local element ids)              8 KB
+    uint16_t inv[kCap];           // inv[rank] = element id                                    8 KB
     uint32_t segstart[kMaxFan + 1];  // tile-local start of every run piece
     uint32_t cur[kMaxFan];        // absolute index of the next unprocessed hit of every run
     uint32_t end[kMaxFan];        // absolute end of every run piece of this tile
-    uint32_t mid[kMaxFan];        // scratch: chunk ends
+    uint32_t mid[kMaxFan];        // scratch: chunk ends (overflow sweep)
+    uint32_t pstart[kCap / 32];   // bitmap of piece starts (run check)
     uint32_t scan[33];
     uint64_t red64[2 * (kMThreads / 32)];
+    uint64_t mbar;                // TMA completion barrier
 };
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D TMA bulk copy global -> shared (16-byte granules), completion counted in bytes on `bar`
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 
 __device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* sm) {
     uint32_t total;
@@ -174,48 +205,50 @@ __device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* sm) {
     return total;
 }
 
-// Sort the chunk [cur_j, mid_j) over the runs j < K (<= kCap hits in total) and write it at out_base.
+__device__ __forceinline__ uint64_t tile_key(const MergeSmem& sm, uint32_t e) {
+    const uint2 v = *reinterpret_cast<const uint2*>(&sm.tile[e]);
+    return (((uint64_t)v.y << 32) | v.x) ^ 0x8000000000000000ull;
+}
+__device__ __forceinline__ uint32_t bucket_start(const MergeSmem& sm, uint32_t b) {
+    return (sm.cnt[b >> 1] >> ((b & 1) * 16)) & 0xFFFFu;
+}
+
+// Sort the chunk [cur_j, chunk_end_j) over the runs j < K (<= kCap hits in total) and write it at out_base.
 // Keys of the chunk lie in [Ta, Ta + width).  Returns the chunk size (uniform over the block).
+// `phase` is the parity of the TMA barrier for this use (flips every call).
 template <bool kPerm>
 __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint4* __restrict__ out, uint32_t K,
                                const uint32_t* chunk_end, uint64_t Ta, uint64_t width, uint32_t out_base,
                                const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out, bool check_runs,
-                               const uint32_t* __restrict__ run_begin, int32_t* __restrict__ status) {
-    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+                               const uint32_t* __restrict__ run_begin, int32_t* __restrict__ status, uint32_t& phase) {
+    const uint32_t tid = threadIdx.x;
     // tile-local piece starts
+    uint32_t my_len = 0, my_s0 = 0;
     {
-        const uint32_t len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
+        my_len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
         uint32_t total;
-        const uint32_t ex = block_exclusive_scan(len, sm.scan, &total);
-        if (tid < K) sm.segstart[tid] = ex;
-        if (tid == 0) sm.segstart[K] = total;
-    }
-    for (uint32_t b = tid; b < (uint32_t)kCap; b += kMThreads) sm.cnt[b] = 0;
-    __syncthreads();
-    const uint32_t count = sm.segstart[K];
-    // stage the pieces: one warp per run, lanes over consecutive records (coalesced 16-byte loads)
-    bool unsorted = false;
-    for (uint32_t j = warp; j < K; j += kMThreads / 32) {
-        const uint32_t a = sm.cur[j], s0 = sm.segstart[j], len = sm.segstart[j + 1] - s0;
-        uint64_t carry_key = 0;
-        bool have_carry = false;
-        if (check_runs && len && a > run_begin[j]) { carry_key = key_at(in, a - 1); have_carry = true; }
-        for (uint32_t p0 = 0; p0 < len; p0 += 32) {
-            const uint32_t p = p0 + lane;
-            uint4 v = make_uint4(0, 0, 0, 0);
-            if (p < len) { v = __ldg(in + a + p); sm.tile[s0 + p] = v; }
-            if (check_runs) {
-                const uint64_t k = key_of(hit_time(v));
-                uint64_t prev = __shfl_up_sync(0xffffffffu, k, 1);
-                bool has_prev = lane > 0;
-                if (lane == 0) { prev = carry_key; has_prev = have_carry; }
-                if (p < len && has_prev && prev > k) unsorted = true;
-                carry_key = __shfl_sync(0xffffffffu, k, 31);
-                have_carry = true;
-            }
+        my_s0 = block_exclusive_scan(my_len, sm.scan, &total);
+        if (tid < K) sm.segstart[tid] = my_s0;
+        if (tid == 0) {
+            sm.segstart[K] = total;
+            if (total) mbar_expect_tx(&sm.mbar, total * 16u);
         }
     }
-    if (check_runs && __syncthreads_or(unsorted) && tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
+    fence_proxy_async();  // earlier generic-proxy accesses of the tile buffer are ordered before the bulk copies
+    __syncthreads();
+    const uint32_t count = sm.segstart[K];
+    // stage the pieces: one TMA bulk copy per run piece, all in flight at once
+    if (my_len) bulk_g2s(&sm.tile[my_s0], in + sm.cur[tid], my_len * 16u, &sm.mbar);
+    // meanwhile: clear the counters and the piece-start bitmap, fetch the run predecessors
+    for (uint32_t b = tid; b < (uint32_t)kCap / 2; b += kMThreads) sm.cnt[b] = 0;
+    if (check_runs && tid < (uint32_t)kCap / 32) sm.pstart[tid] = 0;
+    uint64_t prev_key = 0;
+    bool has_prev = false;
+    if (check_runs && my_len && sm.cur[tid] > run_begin[tid]) { prev_key = key_at(in, sm.cur[tid] - 1); has_prev = true; }
+    __syncthreads();
+    if (check_runs && my_len) atomicOr(&sm.pstart[my_s0 >> 5], 1u << (my_s0 & 31));
+    mbar_wait(&sm.mbar, phase);
+    phase ^= 1u;
     __syncthreads();
     // bucket function: monotone map of (key - Ta) in [0, width) onto [0, kCap)
     int pre = 0;
@@ -223,39 +256,51 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
     const uint32_t wp = (uint32_t)(width >> pre);
     const bool direct = wp <= (uint32_t)kCap;
     const uint32_t scale = direct ? 0u : (uint32_t)(((uint64_t)kCap << 32) / wp);
-    uint32_t bk[kMItems], slot[kMItems];
+    uint32_t bs[kMItems];  // bucket << 16 | slot
+    bool unsorted = false;
+    if (check_runs && has_prev && prev_key > tile_key(sm, my_s0)) unsorted = true;
 #pragma unroll
     for (int i = 0; i < kMItems; ++i) {
         const uint32_t e = tid + i * kMThreads;
-        bk[i] = 0; slot[i] = 0;
+        bs[i] = 0;
         if (e < count) {
-            const uint64_t key = key_of(hit_time(sm.tile[e]));
+            const uint64_t key = tile_key(sm, e);
+            if (check_runs && e > 0 && !((sm.pstart[e >> 5] >> (e & 31)) & 1u) && tile_key(sm, e - 1) > key) unsorted = true;
             uint64_t dt = key - Ta;
             if (key < Ta) dt = 0;
             if (dt >= width) dt = width - 1;
             const uint32_t d = (uint32_t)(dt >> pre);
             uint32_t b = direct ? d : __umulhi(d, scale);
             if (b >= (uint32_t)kCap) b = kCap - 1;
-            bk[i] = b;
-            slot[i] = atomicAdd(&sm.cnt[b], 1u);
+            const uint32_t sh = (b & 1) * 16;
+            const uint32_t old = atomicAdd(&sm.cnt[b >> 1], 1u << sh);
+            bs[i] = (b << 16) | ((old >> sh) & 0xFFFFu);
         }
     }
-    __syncthreads();
-    // exclusive scan of the kCap counters (kMItems consecutive counters per thread)
+    if (check_runs) {
+        if (__syncthreads_or(unsorted) && tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
+    } else {
+        __syncthreads();
+    }
+    // exclusive scan of the kCap packed counters: 8 consecutive counters (one 16-byte word) per thread
     {
-        uint32_t c[kMItems], s = 0;
+        uint4 w = reinterpret_cast<uint4*>(sm.cnt)[tid];
+        uint32_t c[8] = {w.x & 0xFFFFu, w.x >> 16, w.y & 0xFFFFu, w.y >> 16, w.z & 0xFFFFu, w.z >> 16, w.w & 0xFFFFu, w.w >> 16};
+        uint32_t s = 0;
 #pragma unroll
-        for (int i = 0; i < kMItems; ++i) { c[i] = sm.cnt[tid * kMItems + i]; s += c[i]; }
+        for (int i = 0; i < 8; ++i) s += c[i];
         uint32_t total;
         uint32_t ex = block_exclusive_scan(s, sm.scan, &total);
 #pragma unroll
-        for (int i = 0; i < kMItems; ++i) { sm.cnt[tid * kMItems + i] = ex; ex += c[i]; }
+        for (int i = 0; i < 8; ++i) { const uint32_t t = c[i]; c[i] = ex; ex += t; }
+        w.x = c[0] | (c[1] << 16); w.y = c[2] | (c[3] << 16); w.z = c[4] | (c[5] << 16); w.w = c[6] | (c[7] << 16);
+        reinterpret_cast<uint4*>(sm.cnt)[tid] = w;
     }
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < kMItems; ++i) {
         const uint32_t e = tid + i * kMThreads;
-        if (e < count) sm.list[sm.cnt[bk[i]] + slot[i]] = (uint16_t)e;
+        if (e < count) sm.list[bucket_start(sm, bs[i] >> 16) + (bs[i] & 0xFFFFu)] = (uint16_t)e;
     }
     __syncthreads();
     // exact rank inside the bucket: order by (key, element id) = (time, input order)
@@ -263,14 +308,15 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
     for (int i = 0; i < kMItems; ++i) {
         const uint32_t e = tid + i * kMThreads;
         if (e < count) {
-            const uint64_t key = key_of(hit_time(sm.tile[e]));
-            const uint32_t s0 = sm.cnt[bk[i]];
-            const uint32_t s1 = bk[i] + 1 < (uint32_t)kCap ? sm.cnt[bk[i] + 1] : count;
+            const uint32_t b = bs[i] >> 16;
+            const uint32_t s0 = bucket_start(sm, b);
+            const uint32_t s1 = b + 1 < (uint32_t)kCap ? bucket_start(sm, b + 1) : count;
             uint32_t r = s0;
-            for (uint32_t m = s0; m < s1; ++m) {
-                const uint32_t o = sm.list[m];
-                if (o != e) {
-                    const uint64_t ko = key_of(hit_time(sm.tile[o]));
+            if (s1 - s0 > 1) {
+                const uint64_t key = tile_key(sm, e);
+                for (uint32_t m = s0; m < s1; ++m) {
+                    const uint32_t o = sm.list[m];
+                    const uint64_t ko = tile_key(sm, o);
                     r += (ko < key || (ko == key && o < e)) ? 1u : 0u;
                 }
             }
@@ -302,10 +348,9 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     extern __shared__ __align__(16) unsigned char smem_raw[];
     MergeSmem& sm = *reinterpret_cast<MergeSmem*>(smem_raw);
     const uint32_t tid = threadIdx.x;
-    // which (group, tile)?
-    uint32_t lo = 0, hi = lv.G;
-    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (lv.tbase[mid] <= blockIdx.x) lo = mid; else hi = mid; }
-    const uint32_t g = lo, k = blockIdx.x - lv.tbase[g];
+    if (tid == 0) mbar_init(&sm.mbar, 1);
+    uint32_t phase = 0;
+    const uint32_t g = lv.tile_g[blockIdx.x], k = blockIdx.x - lv.tbase[g];
     const uint32_t r0 = lv.gfirst[g], K = lv.gfirst[g + 1] - r0;
     const uint32_t nt = lv.tbase[g + 1] - lv.tbase[g];
     const uint32_t* row0 = lv.splits + lv.sbase[g] + (size_t)k * K;
@@ -330,7 +375,7 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     (void)nt;
     if (remaining <= (uint32_t)kCap) {  // the common case: the whole tile in one chunk
         if (remaining)
-            sort_chunk<kPerm>(sm, in, out, K, sm.end, Ta, DT, out_base, perm_in, perm_out, check_runs != 0, run_begin, status);
+            sort_chunk<kPerm>(sm, in, out, K, sm.end, Ta, DT, out_base, perm_in, perm_out, check_runs != 0, run_begin, status, phase);
         return;
     }
     // ---- overflow sweep: chunks of <= kCap hits in key order ------------------------------------------
@@ -354,7 +399,7 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
         __syncthreads();
         if (remaining <= (uint32_t)kCap) {
             const uint32_t c = sort_chunk<kPerm>(sm, in, out, K, sm.end, kmin, kmax - kmin + 1 ? kmax - kmin + 1 : ~0ull,
-                                                 out_base, perm_in, perm_out, check_runs != 0, run_begin, status);
+                                                 out_base, perm_in, perm_out, check_runs != 0, run_begin, status, phase);
             out_base += c;
             break;
         }
@@ -394,7 +439,7 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
         const uint32_t ex = block_exclusive_scan(c, sm.scan, &total);
         if (have_lo && total) {
             sort_chunk<kPerm>(sm, in, out, K, sm.mid, kmin, xlo - kmin + 1, out_base, perm_in, perm_out, check_runs != 0,
-                              run_begin, status);
+                              run_begin, status, phase);
         } else {
             // tie block: every hit has key == kmin; the stable order is the run-major concatenation
             if (tid < K) sm.segstart[tid] = ex;
@@ -500,6 +545,7 @@ static void carve(Arena& a, const std::vector<LevelHost>& levels, uint32_t n, bo
         d.gDT = a.take<uint64_t>(L.G + 1);
         d.splits = a.take<uint32_t>((size_t)L.split_entries + 1);
         d.roff_next = a.take<uint32_t>(L.G + 1);
+        d.tile_g = a.take<uint32_t>((size_t)L.tiles + 1);
     }
     const size_t nlev = levels.size();
     w.tmp[0] = nlev > 1 ? a.take<uint4>(n) : nullptr;
