@@ -232,6 +232,8 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (device time from the stage events of the timed steps) ----
     peak, peak_src = peaks()
+    counters = {k[4:]: v[0] / max(v[1], 1) for k, v in stages.items() if k.startswith("ctr.")}
+    stages = {k: v for k, v in stages.items() if not k.startswith("ctr.")}
     per_stage = {k: v[0] / args.steps for k, v in stages.items()}  # ms per step
     dom = max(per_stage, key=per_stage.get) if per_stage else None
     roof = None
@@ -318,6 +320,7 @@ def run_ours(args):
             "pipeline_roofline": {"alg_bytes_per_hit": ALG_BYTES_PIPELINE, "achieved": pipe_ach, "peak": peak,
                                   "unit": "GB/s", "frac": pipe_ach / peak},
             "stages_ms_per_step": {k: round(v, 5) for k, v in sorted(per_stage.items())},
+            "counters": counters,
             "e2e": e2e, "cpu_baseline": cpu,
         }
         print(json.dumps(out))

@@ -27,6 +27,7 @@ void count_launch();                                // every kernel launch of th
 void prof_mark(cudaStream_t s, const char* name);   // no-op unless tt_prof_enable(1): records an event that
                                                     // opens stage `name` (and closes the previous one)
 void prof_end(cudaStream_t s);                      // closes the current stage
+void prof_counter(cudaStream_t s, const char* name, const uint32_t* d_value);  // samples a device counter (profiling only)
 #define TT_K(k) tt::count_launch(), k
 
 struct tt_geometry_dev {  // device view of the causality table

@@ -36,6 +36,21 @@ static void mark(cudaStream_t s, const char* name) {
     g_marks.push_back({e, name});
 }
 void prof_mark(cudaStream_t s, const char* name) { mark(s, name); }
+
+// device counters sampled while profiling: copied to pinned host memory on the caller's stream
+struct Counter {
+    const char* name;
+    uint32_t* host;  // pinned
+};
+static std::vector<Counter> g_counters;
+void prof_counter(cudaStream_t s, const char* name, const uint32_t* d_value) {
+    if (!g_on || g_counters.size() >= 4096) return;
+    uint32_t* h = nullptr;
+    if (cudaMallocHost(&h, sizeof(uint32_t)) != cudaSuccess) return;
+    *h = 0;
+    cudaMemcpyAsync(h, d_value, sizeof(uint32_t), cudaMemcpyDeviceToHost, s);
+    g_counters.push_back({name, h});
+}
 void prof_end(cudaStream_t s) { mark(s, nullptr); }
 }  // namespace tt
 
@@ -45,6 +60,8 @@ extern "C" int tt_prof_enable(int on) {
     tt::g_on = on != 0;
     tt::g_marks.clear();
     tt::g_used = 0;
+    for (auto& c : tt::g_counters) cudaFreeHost(c.host);
+    tt::g_counters.clear();
     return TT_OK;
 }
 
@@ -67,6 +84,15 @@ extern "C" int tt_prof_read(char* buf, size_t cap) {
             if (names[j] == g_marks[k].name) break;
         if (j == names.size()) { names.push_back(g_marks[k].name); ms.push_back(0); cnt.push_back(0); }
         ms[j] += t;
+        cnt[j] += 1;
+    }
+    for (auto& c : g_counters) {  // counters: "ctr.<name> <sum of values> <samples>"
+        const std::string nm = std::string("ctr.") + c.name;
+        size_t j = 0;
+        for (; j < names.size(); ++j)
+            if (names[j] == nm) break;
+        if (j == names.size()) { names.push_back(nm); ms.push_back(0); cnt.push_back(0); }
+        ms[j] += (double)*c.host;
         cnt[j] += 1;
     }
     size_t off = 0;

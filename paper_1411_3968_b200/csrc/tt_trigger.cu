@@ -11,9 +11,18 @@
 namespace tt {
 
 // ------------------------------------------------------------------------------------------------
-// L1: one thread per hit, neighbours read through L1/L2 cache (adjacent records).
+// L1.  One CTA per tile of kL1Tile consecutive sorted hits, staged in shared memory (with a halo of
+// kL1Halo hits on both sides) as (32-bit time relative to the first staged hit, floor << 16 | pmt).
+// Every staged hit scans FORWARD while t_j - t_i <= LC and marks both partners of a same-floor /
+// other-PMT pair, so each pair is tested once.  What the staged window cannot decide (a neighbourhood
+// reaching past the halo, a tile spanning >= 2^32 ps, a segment boundary) is finished by exact scans
+// of global memory, so the result is the plain definition for any input.
 // ------------------------------------------------------------------------------------------------
 constexpr int kL1Threads = 256;
+constexpr int kL1Per = 16;                        // in-tile hits per thread
+constexpr int kL1Tile = kL1Threads * kL1Per;      // 4096
+constexpr int kL1Halo = kL1Threads;               // staged hits before and after the tile
+constexpr int kL1Stage = kL1Tile + 2 * kL1Halo;   // 4608
 
 struct L1Rec {  // compact L1 hit, 16 bytes
     int64_t t;
@@ -22,62 +31,210 @@ struct L1Rec {  // compact L1 hit, 16 bytes
 };
 constexpr uint32_t kBadTp = 0xFFFFFFFFu;
 
-__global__ void __launch_bounds__(kL1Threads) l1_flags_kernel(const uint4* __restrict__ hits, uint32_t n,
-                                                              const uint32_t* __restrict__ seg_off, uint32_t n_seg,
-                                                              uint64_t lc, uint32_t q_thresh,
-                                                              uint8_t* __restrict__ flags,
-                                                              uint32_t* __restrict__ blk_cnt) {
-    const uint32_t i = blockIdx.x * kL1Threads + threadIdx.x;
-    uint32_t f = 0;
-    if (i < n) {
-        const HitView h = unpack(__ldg(hits + i));
-        uint32_t a = 0, b = n;
-        if (n_seg > 1) {
-            const uint32_t s = find_segment(seg_off, n_seg, i);
-            a = __ldg(seg_off + s);
-            b = __ldg(seg_off + s + 1);
-        }
-        if (h.charge >= q_thresh) f |= TT_Q;
-        bool lcb = false;
-        for (uint32_t j = i; j > a && !lcb;) {
-            --j;
-            const HitView o = unpack(__ldg(hits + j));
-            if (udiff(h.t, o.t) > lc) break;
-            lcb = (o.floor == h.floor) & (o.pmt != h.pmt);
-        }
-        for (uint32_t j = i + 1; j < b && !lcb; ++j) {
-            const HitView o = unpack(__ldg(hits + j));
-            if (udiff(o.t, h.t) > lc) break;
-            lcb = (o.floor == h.floor) & (o.pmt != h.pmt);
-        }
-        if (lcb) f |= TT_LC;
-        if (f) f |= TT_L1;
-        flags[i] = (uint8_t)f;
+// exact LC bit of hit i by scanning global memory outwards from (below, above): partners j < below and
+// j >= above inside [a, b)
+__device__ __forceinline__ bool lc_scan_global(const uint4* __restrict__ hits, int64_t t, uint32_t fp, uint32_t below,
+                                               uint32_t above, uint32_t a, uint32_t b, uint64_t lc) {
+    for (uint32_t j = below; j > a;) {
+        --j;
+        const uint4 v = __ldg(hits + j);
+        if (udiff(t, hit_time(v)) > lc) break;
+        const uint32_t x = v.z ^ fp;
+        if (x - 1u < 0xFFFFu) return true;  // same floor (high half equal), other pmt (low half differs)
     }
-    const int c = __syncthreads_count(f != 0);
-    if (threadIdx.x == 0) blk_cnt[blockIdx.x] = (uint32_t)c;
+    for (uint32_t j = above; j < b; ++j) {
+        const uint4 v = __ldg(hits + j);
+        if (udiff(hit_time(v), t) > lc) break;
+        const uint32_t x = v.z ^ fp;
+        if (x - 1u < 0xFFFFu) return true;
+    }
+    return false;
 }
 
-// ordered compaction of the L1 hits (block offsets from the scan of blk_cnt)
+constexpr int kL1Pad = 64;  // readable slack behind the staged arrays (speculative key reads)
+
+__global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __restrict__ hits, uint32_t n,
+                                                             const uint32_t* __restrict__ seg_off, uint32_t n_seg,
+                                                             uint64_t lc, uint32_t q_thresh,
+                                                             uint8_t* __restrict__ flags,
+                                                             uint32_t* __restrict__ tile_cnt) {
+    __shared__ uint32_t s_t[kL1Stage + kL1Pad];   // time relative to the first staged hit
+    __shared__ uint32_t s_k[kL1Stage + kL1Pad];   // floor << 16 | pmt
+    __shared__ __align__(16) uint32_t s_f[kL1Tile / 4];  // flag bytes of the in-tile hits
+    __shared__ uint32_t s_red[kL1Threads / 32];
+    const uint32_t tid = threadIdx.x, lane = tid & 31;
+    const uint32_t tb = blockIdx.x * (uint32_t)kL1Tile;                 // first in-tile hit
+    const uint32_t te = min(n, tb + (uint32_t)kL1Tile);                 // end of the tile
+    const uint32_t glo = tb >= (uint32_t)kL1Halo ? tb - kL1Halo : 0u;   // first staged hit
+    const uint32_t ghi = min(n, te + (uint32_t)kL1Halo);                // end of the staged hits
+    // staged slot e <-> global index g0 + e (g0 = tb - kL1Halo, modulo 2^32); slot kL1Halo = first in-tile hit
+    const uint32_t g0 = tb - (uint32_t)kL1Halo;
+    const uint32_t e_lo = glo - g0, e_hi = ghi - g0, e_te = te - g0;
+    uint32_t seg_a = 0, seg_b = n;
+    bool one_seg = true;
+    if (n_seg > 1) {
+        const uint32_t s = find_segment(seg_off, n_seg, glo);
+        seg_a = __ldg(seg_off + s);
+        seg_b = __ldg(seg_off + s + 1);
+        one_seg = seg_b >= ghi;
+    }
+    const int64_t t0 = hit_time(__ldg(hits + glo));
+    const uint64_t span = udiff(hit_time(__ldg(hits + (ghi - 1))), t0);
+    const bool fits32 = span < 0xFFFFFFFFull;  // every staged time is t0 + (a 32-bit offset)
+    uint8_t* s_fb = reinterpret_cast<uint8_t*>(s_f);
+#pragma unroll
+    for (int k = 0; k < kL1Per + 2; ++k) {
+        const uint32_t e = tid + k * kL1Threads;
+        uint32_t tr = 0xFFFFFFFFu, ky = 0xFFFFFFFFu, q = 0;
+        if (e >= e_lo && e < e_hi) {
+            const uint4 v = __ldg(hits + (g0 + e));
+            tr = (uint32_t)udiff(hit_time(v), t0);
+            ky = v.z;
+            q = (v.w & 0xFFFFu) >= q_thresh ? (uint32_t)TT_Q : 0u;
+        }
+        s_t[e] = tr;
+        s_k[e] = ky;
+        if (k >= 1 && k <= kL1Per) s_fb[e - kL1Halo] = (uint8_t)q;
+    }
+    if (tid < kL1Pad) { s_t[kL1Stage + tid] = 0xFFFFFFFFu; s_k[kL1Stage + tid] = 0xFFFFFFFFu; }
+    __syncthreads();
+    const uint32_t lc32 = lc > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)lc;
+    if (fits32) {
+        const uint32_t t_last = s_t[e_hi - 1];
+        // chunk k = 0: the halo before the tile (marks its in-tile partners only); k = 1..16: the tile
+#pragma unroll 1
+        for (int k = 0; k <= kL1Per; ++k) {
+            const uint32_t e = tid + k * kL1Threads;
+            const uint32_t w0 = e - lane;                       // first slot of this warp's chunk
+            if (w0 >= e_te) break;                              // warp-uniform
+            const bool valid = e >= e_lo && e < e_te;
+            const uint32_t ti = s_t[e], ki = s_k[e];
+            uint32_t jmax = e_hi, sa = seg_a, sb = seg_b;
+            if (!one_seg && valid) {
+                const uint32_t s = find_segment(seg_off, n_seg, g0 + e);
+                sa = __ldg(seg_off + s);
+                sb = __ldg(seg_off + s + 1);
+                if (sb < ghi) jmax = sb - g0;
+            }
+            bool found = false;
+            const uint32_t dmax = e_hi - w0;                    // warp-uniform bound on the offsets
+            for (uint32_t d0 = 1; d0 < dmax; d0 += 4) {
+                // does any hit of the chunk still have offset d0 inside its window?
+                if (!__any_sync(0xffffffffu, valid && (s_t[e + d0] - ti <= lc32))) break;
+#pragma unroll
+                for (uint32_t q = 0; q < 4; ++q) {
+                    const uint32_t j = e + d0 + q;
+                    const uint32_t x = s_k[j] ^ ki;
+                    if (x - 1u < 0xFFFFu) {                     // same floor, other PMT: rare; now the exact tests
+                        if (valid && j < jmax && s_t[j] - ti <= lc32) {
+                            found = true;
+                            if (j >= (uint32_t)kL1Halo && j < e_te)
+                                atomicOr(&s_f[(j - kL1Halo) >> 2], (uint32_t)TT_LC << (8 * ((j - kL1Halo) & 3)));
+                        }
+                    }
+                }
+            }
+            if (k == 0 || !valid) continue;
+            // what the staged window leaves open: partners beyond its end / before its start
+            const bool open_fwd = jmax == e_hi && ghi < sb && t_last - ti <= lc32;
+            const bool open_bwd = max(glo, sa) > sa && (uint64_t)ti <= lc;  // the first staged hit is inside the window
+            if (!found && (open_fwd || open_bwd)) {
+                const int64_t t = (int64_t)((uint64_t)t0 + ti);
+                found = lc_scan_global(hits, t, ki, open_bwd ? glo : sa, open_fwd ? ghi : sb, sa, sb, lc);
+            }
+            if (found) atomicOr(&s_f[(e - kL1Halo) >> 2], (uint32_t)TT_LC << (8 * ((e - kL1Halo) & 3)));
+        }
+    } else {
+        // ---- sparse tile (>= 2^32 ps across the staged hits): exact scans of global memory ------------
+#pragma unroll 1
+        for (int k = 1; k <= kL1Per; ++k) {
+            const uint32_t e = tid + k * kL1Threads;
+            if (e >= e_te) break;
+            const uint32_t g = g0 + e;
+            uint32_t sa = seg_a, sb = seg_b;
+            if (!one_seg) {
+                const uint32_t s = find_segment(seg_off, n_seg, g);
+                sa = __ldg(seg_off + s);
+                sb = __ldg(seg_off + s + 1);
+            }
+            const uint4 v = __ldg(hits + g);
+            if (lc_scan_global(hits, hit_time(v), v.z, g, g + 1, sa, sb, lc))
+                atomicOr(&s_f[(e - kL1Halo) >> 2], (uint32_t)TT_LC << (8 * ((e - kL1Halo) & 3)));
+        }
+    }
+    __syncthreads();
+    // thread t writes the 16 flag bytes [16 t, 16 t + 16) of the tile: L1 = Q | LC
+    uint32_t cnt = 0;
+    {
+        uint4 v = reinterpret_cast<const uint4*>(s_f)[tid];
+        uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const uint32_t any = (w[q] | (w[q] >> 1)) & 0x01010101u;  // Q = 1, LC = 2
+            w[q] |= any << 2;                                          // L1 = 4
+            cnt += __popc(any);
+        }
+        const uint32_t i0 = tb + tid * 16u;
+        if (i0 + 16u <= te && (((uintptr_t)(flags + i0)) & 15) == 0) {
+            *reinterpret_cast<uint4*>(flags + i0) = make_uint4(w[0], w[1], w[2], w[3]);
+        } else {
+            cnt = 0;
+            for (uint32_t b8 = 0; b8 < 16u && i0 + b8 < te; ++b8) {
+                const uint32_t f = (w[b8 >> 2] >> (8 * (b8 & 3))) & 0xFFu;
+                flags[i0 + b8] = (uint8_t)f;
+                cnt += f ? 1u : 0u;
+            }
+        }
+    }
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    if (lane == 0) s_red[tid >> 5] = cnt;
+    __syncthreads();
+    if (tid == 0) {
+        uint32_t c = 0;
+#pragma unroll
+        for (int w = 0; w < kL1Threads / 32; ++w) c += s_red[w];
+        tile_cnt[blockIdx.x] = c;
+    }
+}
+
+// ordered compaction of the L1 hits, one CTA per L1 tile (tile offsets from the scan of tile_cnt):
+// thread t owns the 16 consecutive flag bytes [16 t, 16 t + 16) of the tile.
 __global__ void __launch_bounds__(kL1Threads) l1_compact_kernel(const uint4* __restrict__ hits, uint32_t n,
                                                                 const uint8_t* __restrict__ flags,
-                                                                const uint32_t* __restrict__ blk_off,
+                                                                const uint32_t* __restrict__ tile_off,
                                                                 L1Rec* __restrict__ l1, uint32_t n_pmt, uint32_t ppt,
                                                                 int32_t* __restrict__ status) {
     __shared__ uint32_t sm[33];
-    const uint32_t i = blockIdx.x * kL1Threads + threadIdx.x;
-    const bool is = i < n && (flags[i] & TT_L1);
+    const uint32_t i0 = blockIdx.x * (uint32_t)kL1Tile + threadIdx.x * kL1Per;
+    uint32_t mask = 0;
+    if (i0 < n) {
+        if (i0 + kL1Per <= n && (((uintptr_t)(flags + i0)) & 15) == 0) {
+            const uint4 v = *reinterpret_cast<const uint4*>(flags + i0);
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int b8 = 0; b8 < 4; ++b8)
+                    if ((w[q] >> (8 * b8)) & TT_L1) mask |= 1u << (q * 4 + b8);
+        } else {
+            for (uint32_t k = 0; k < (uint32_t)kL1Per && i0 + k < n; ++k)
+                if (flags[i0 + k] & TT_L1) mask |= 1u << k;
+        }
+    }
     uint32_t total;
-    const uint32_t r = block_exclusive_scan(is ? 1u : 0u, sm, &total);
+    uint32_t r = tile_off[blockIdx.x] + block_exclusive_scan(__popc(mask), sm, &total);
     bool bad = false;
-    if (is) {
+    while (mask) {
+        const uint32_t k = __ffs(mask) - 1;
+        mask &= mask - 1;
+        const uint32_t i = i0 + k;
         const HitView h = unpack(__ldg(hits + i));
         L1Rec rec;
         rec.t = h.t;
         rec.idx = i;
         if (h.pmt >= n_pmt) { rec.tp = kBadTp; bad = true; }
         else { const uint32_t tw = h.pmt / ppt; rec.tp = (tw << 16) | (h.pmt - tw * ppt); }
-        l1[blk_off[blockIdx.x] + r] = rec;
+        l1[r++] = rec;
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(status, TT_S_BAD_PMT);
 }
@@ -521,7 +678,7 @@ struct TriggerPlan {
 };
 
 static void trigger_plan(Arena& a, uint32_t n, TriggerPlan& p) {
-    p.nblk = div_up(n, kL1Threads);
+    p.nblk = div_up(n, kL1Tile);
     p.blk_cnt = a.take<uint32_t>(p.nblk + 1);
     p.scan_scratch = a.take<uint32_t>(scan_ws_count(p.nblk + 1));
     p.m_total = a.take<uint32_t>(1);
@@ -574,8 +731,8 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
         attr_done = true;
     }
     prof_mark(s, "trig.l1_flags");
-    TT_K(l1_flags_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,
-                                                     (uint64_t)p->lc_window_ps, p->q_thresh, d_flags, plan.blk_cnt);
+    TT_K(l1_tile_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,
+                                                    (uint64_t)p->lc_window_ps, p->q_thresh, d_flags, plan.blk_cnt);
     prof_mark(s, "trig.l1_scan");
     int rc = exclusive_scan_u32(plan.blk_cnt, plan.blk_cnt, plan.nblk, plan.scan_scratch, plan.m_total, s);
     if (rc != TT_OK) return rc;
@@ -594,6 +751,8 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     TT_K(l2_wide_kernel)<<<kSMs * 4, kL2Warps * 32, sizeof(WideSmem) * kL2Warps, s>>>(
         plan.l1, plan.m_total, plan.slow_list, plan.slow_cnt, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps,
         p->l2_multiplicity, p->l2_mode, d_flags, plan.l2bit, d_status);
+    prof_counter(s, "l1_hits", plan.m_total);
+    prof_counter(s, "l2_slow_items", plan.slow_cnt);
     prof_mark(s, "trig.seeds");
     TT_K(seed_count_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.m_total, plan.seed_cnt);
     TT_K(count_scan_kernel)<<<1, 1024, 0, s>>>(plan.seed_cnt, kSeedBlocks, d_n_seeds, seed_cap, TT_S_SEED_OVERFLOW, d_status);
