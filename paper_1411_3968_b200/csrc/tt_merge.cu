@@ -139,8 +139,10 @@ __global__ void __launch_bounds__(256) merge_partition_kernel(LevelDev lv, const
     const uint32_t g = lo;
     const uint32_t r0 = lv.gfirst[g], K = lv.gfirst[g + 1] - r0;
     const uint32_t local = id - lv.sbase[g];
-    const uint32_t k = local / K, j = local - k * K;
     const uint32_t nt = lv.tbase[g + 1] - lv.tbase[g];
+    // consecutive threads take consecutive boundaries k of ONE run j: their searches share the upper levels
+    // and end in neighbouring cache lines (the table itself stays [k][j], as the tile kernel reads it)
+    const uint32_t j = local / (nt + 1), k = local - j * (nt + 1);
     uint32_t a = lv.roff[r0 + j], b = lv.roff[r0 + j + 1];
     uint32_t res;
     if (k == 0) res = a;
@@ -152,16 +154,16 @@ __global__ void __launch_bounds__(256) merge_partition_kernel(LevelDev lv, const
         while (a < b) { const uint32_t mid = a + ((b - a) >> 1); if (key_at(hits, mid) < T) a = mid + 1; else b = mid; }
         res = a;
     }
-    lv.splits[id] = res;
+    lv.splits[lv.sbase[g] + (size_t)k * K + j] = res;
     if (j == 0 && k < nt) lv.tile_g[lv.tbase[g] + k] = g;
 }
 
 // ---- the tile kernel ---------------------------------------------------------------------------------
 struct MergeSmem {
     uint4 tile[kCap];             // staged records, run-major (filled by TMA bulk copies)   64 KB
-    uint32_t cnt[kCap / 2];       // packed 16-bit bucket counters -> exclusive starts         8 KB
-    uint16_t list[kCap];          // bucket member lists (tile-local element ids)              8 KB
-    uint16_t inv[kCap];           // inv[rank] = element id                                    8 KB
+    uint32_t cs[kCap];            // 32-bit-key path: per bucket start << 16 | count, later inv[] (u16)      16 KB
+                                  // wide-key path:   packed 16-bit counters (8 KB) + inv[] (u16, 8 KB)
+    uint32_t list[kCap];          // 32-bit-key path: bucket member composites; wide-key path: member ids (u16)  16 KB
     uint32_t segstart[kMaxFan + 1];  // tile-local start of every run piece
     uint32_t cur[kMaxFan];        // absolute index of the next unprocessed hit of every run
     uint32_t end[kMaxFan];        // absolute end of every run piece of this tile
@@ -171,6 +173,7 @@ struct MergeSmem {
     uint64_t red64[2 * (kMThreads / 32)];
     uint64_t mbar;                // TMA completion barrier
 };
+static_assert(2 * (sizeof(MergeSmem) + 1024) <= 233472, "two CTAs per SM");
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
@@ -210,7 +213,154 @@ __device__ __forceinline__ uint64_t tile_key(const MergeSmem& sm, uint32_t e) {
     return (((uint64_t)v.y << 32) | v.x) ^ 0x8000000000000000ull;
 }
 __device__ __forceinline__ uint32_t bucket_start(const MergeSmem& sm, uint32_t b) {
-    return (sm.cnt[b >> 1] >> ((b & 1) * 16)) & 0xFFFFu;
+    return (sm.cs[b >> 1] >> ((b & 1) * 16)) & 0xFFFFu;
+}
+
+// ---- 32-bit-key chunk sort (the common case: the chunk spans < 2^32 ps) -----------------------------------
+// Same contract as sort_chunk below.  Counting sort on kCap fine buckets of the 32-bit key offset d = key - Ta:
+// bucket = hi32(d * scale), and the top 20 bits of lo32(d * scale) order the keys inside a bucket exactly
+// (scale >= 2^12, so two different offsets of one bucket differ there); with the 12-bit element id below them
+// one 32-bit composite per hit gives the stable order by a single unsigned compare.
+template <bool kPerm>
+__device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, uint4* __restrict__ out, uint32_t K,
+                                 const uint32_t* chunk_end, uint64_t Ta, uint32_t width, uint32_t out_base,
+                                 const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out, bool check_runs,
+                                 const uint32_t* __restrict__ run_begin, int32_t* __restrict__ status, uint32_t& phase) {
+    const uint32_t tid = threadIdx.x, lane = tid & 31;
+    uint32_t my_len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
+    uint32_t total;
+    const uint32_t my_s0 = block_exclusive_scan(my_len, sm.scan, &total);
+    if (tid < K) sm.segstart[tid] = my_s0;
+    if (tid == 0) {
+        sm.segstart[K] = total;
+        if (total) mbar_expect_tx(&sm.mbar, total * 16u);
+    }
+    fence_proxy_async();  // earlier generic-proxy accesses of the tile buffer are ordered before the bulk copies
+    __syncthreads();
+    const uint32_t count = total;
+    // stage the pieces: one TMA bulk copy per run piece, all in flight at once
+    if (my_len) bulk_g2s(&sm.tile[my_s0], in + sm.cur[tid], my_len * 16u, &sm.mbar);
+    // meanwhile: clear the buckets and the piece-start bitmap, fetch the run predecessors
+    {
+        uint4* z = reinterpret_cast<uint4*>(sm.cs);
+#pragma unroll
+        for (int i = 0; i < kCap / 4 / kMThreads; ++i) z[tid + i * kMThreads] = make_uint4(0, 0, 0, 0);
+    }
+    if (check_runs && tid < (uint32_t)kCap / 32) sm.pstart[tid] = 0;
+    uint64_t prev_key = 0;
+    bool has_prev = false;
+    if (check_runs && my_len && sm.cur[tid] > run_begin[tid]) { prev_key = key_at(in, sm.cur[tid] - 1); has_prev = true; }
+    __syncthreads();
+    if (check_runs && my_len) atomicOr(&sm.pstart[my_s0 >> 5], 1u << (my_s0 & 31));
+    mbar_wait(&sm.mbar, phase);
+    phase ^= 1u;
+    __syncthreads();
+    const bool direct = width <= (uint32_t)kCap;
+    const uint32_t scale = direct ? 0u : (uint32_t)(((uint64_t)kCap << 32) / width);
+    const uint32_t Ta_lo = (uint32_t)Ta, Ta_hi = (uint32_t)(Ta >> 32);
+    uint32_t fb[kMItems];    // composite high part (20 bits) << 12 | bucket
+    uint32_t slot[kMItems];  // arrival position in the bucket, later start << 16 | count of the bucket
+    bool unsorted = false;
+    if (check_runs && has_prev && prev_key > tile_key(sm, my_s0)) unsorted = true;
+#pragma unroll
+    for (int i = 0; i < kMItems; ++i) {
+        const uint32_t e = tid + i * kMThreads;
+        fb[i] = 0; slot[i] = 0;
+        uint32_t d = 0;
+        bool oob = false;
+        if (e < count) {
+            const uint2 v = *reinterpret_cast<const uint2*>(&sm.tile[e]);
+            const uint32_t hi = (v.y ^ 0x80000000u) - Ta_hi - (v.x < Ta_lo ? 1u : 0u);  // high word of key - Ta
+            d = v.x - Ta_lo;
+            oob = hi != 0u || d >= width;          // only with unsorted runs (the splits assume sorted runs)
+            if (oob) d = (hi & 0x80000000u) ? 0u : width - 1u;
+        }
+        if (check_runs) {
+            const uint32_t dp = __shfl_up_sync(0xffffffffu, d, 1);
+            if (e < count && e > 0 && !((sm.pstart[e >> 5] >> (e & 31)) & 1u)) {
+                uint32_t pv = dp;
+                if (lane == 0) {  // predecessor held by another warp: recompute its offset
+                    const uint2 u = *reinterpret_cast<const uint2*>(&sm.tile[e - 1]);
+                    const uint32_t uh = (u.y ^ 0x80000000u) - Ta_hi - (u.x < Ta_lo ? 1u : 0u);
+                    pv = u.x - Ta_lo;
+                    if (uh != 0u || pv >= width) pv = (uh & 0x80000000u) ? 0u : width - 1u;
+                }
+                if (pv > d) unsorted = true;
+            }
+            if (oob) unsorted = true;
+        }
+        if (e < count) {
+            uint32_t b, fr;
+            if (direct) { b = d; fr = 0; }
+            else { const uint64_t pr = (uint64_t)d * scale; b = (uint32_t)(pr >> 32); fr = (uint32_t)pr & 0xFFFFF000u; }
+            slot[i] = atomicAdd(&sm.cs[b], 1u) & 0xFFFFu;
+            fb[i] = fr | b;
+        }
+    }
+    if (check_runs) {
+        if (__syncthreads_or(unsorted) && tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
+    } else {
+        __syncthreads();
+    }
+    // exclusive scan of the kCap bucket counts: 8 consecutive buckets per thread -> start << 16 | count
+    {
+        uint4* c4 = reinterpret_cast<uint4*>(sm.cs);
+        uint4 w0 = c4[2 * tid], w1 = c4[2 * tid + 1];
+        uint32_t c[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
+        uint32_t sum = 0;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) sum += c[i];
+        uint32_t tot;
+        uint32_t ex = block_exclusive_scan(sum, sm.scan, &tot);
+#pragma unroll
+        for (int i = 0; i < 8; ++i) { const uint32_t t = c[i]; c[i] = (ex << 16) | t; ex += t; }
+        c4[2 * tid] = make_uint4(c[0], c[1], c[2], c[3]);
+        c4[2 * tid + 1] = make_uint4(c[4], c[5], c[6], c[7]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int i = 0; i < kMItems; ++i) {
+        const uint32_t e = tid + i * kMThreads;
+        if (e < count) {
+            const uint32_t w = sm.cs[fb[i] & 0xFFFu];
+            sm.list[(w >> 16) + slot[i]] = (fb[i] & 0xFFFFF000u) | e;
+            slot[i] = w;
+        }
+    }
+    __syncthreads();
+    // exact rank inside the bucket; inv[] reuses the bucket array (its contents now live in slot[])
+    uint16_t* const inv16 = reinterpret_cast<uint16_t*>(sm.cs);
+#pragma unroll
+    for (int i = 0; i < kMItems; ++i) {
+        const uint32_t e = tid + i * kMThreads;
+        if (e < count) {
+            const uint32_t s0 = slot[i] >> 16, cb = slot[i] & 0xFFFFu;
+            uint32_t r = s0;
+            if (cb > 1u) {
+                const uint32_t c = (fb[i] & 0xFFFFF000u) | e;
+                for (uint32_t m = s0; m < s0 + cb; ++m) r += sm.list[m] < c ? 1u : 0u;
+            }
+            inv16[r] = (uint16_t)e;  // cs[] was last read before the barrier above
+        }
+    }
+    __syncthreads();
+    // coalesced output
+#pragma unroll
+    for (int i = 0; i < kMItems; ++i) {
+        const uint32_t r = tid + i * kMThreads;
+        if (r < count) {
+            const uint32_t e = inv16[r];
+            out[out_base + r] = sm.tile[e];
+            if (kPerm) {
+                uint32_t lo = 0, hi = K;  // piece j with segstart[j] <= e < segstart[j+1]
+                while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (sm.segstart[mid] <= e) lo = mid; else hi = mid; }
+                const uint32_t src = sm.cur[lo] + (e - sm.segstart[lo]);
+                perm_out[out_base + r] = perm_in ? perm_in[src] : src;
+            }
+        }
+    }
+    __syncthreads();
+    return count;
 }
 
 // Sort the chunk [cur_j, chunk_end_j) over the runs j < K (<= kCap hits in total) and write it at out_base.
@@ -240,7 +390,9 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
     // stage the pieces: one TMA bulk copy per run piece, all in flight at once
     if (my_len) bulk_g2s(&sm.tile[my_s0], in + sm.cur[tid], my_len * 16u, &sm.mbar);
     // meanwhile: clear the counters and the piece-start bitmap, fetch the run predecessors
-    for (uint32_t b = tid; b < (uint32_t)kCap / 2; b += kMThreads) sm.cnt[b] = 0;
+    uint16_t* const list16 = reinterpret_cast<uint16_t*>(sm.list);
+    uint16_t* const inv16 = reinterpret_cast<uint16_t*>(sm.cs + kCap / 2);
+    for (uint32_t b = tid; b < (uint32_t)kCap / 2; b += kMThreads) sm.cs[b] = 0;
     if (check_runs && tid < (uint32_t)kCap / 32) sm.pstart[tid] = 0;
     uint64_t prev_key = 0;
     bool has_prev = false;
@@ -273,7 +425,7 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
             uint32_t b = direct ? d : __umulhi(d, scale);
             if (b >= (uint32_t)kCap) b = kCap - 1;
             const uint32_t sh = (b & 1) * 16;
-            const uint32_t old = atomicAdd(&sm.cnt[b >> 1], 1u << sh);
+            const uint32_t old = atomicAdd(&sm.cs[b >> 1], 1u << sh);
             bs[i] = (b << 16) | ((old >> sh) & 0xFFFFu);
         }
     }
@@ -284,7 +436,7 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
     }
     // exclusive scan of the kCap packed counters: 8 consecutive counters (one 16-byte word) per thread
     {
-        uint4 w = reinterpret_cast<uint4*>(sm.cnt)[tid];
+        uint4 w = reinterpret_cast<uint4*>(sm.cs)[tid];
         uint32_t c[8] = {w.x & 0xFFFFu, w.x >> 16, w.y & 0xFFFFu, w.y >> 16, w.z & 0xFFFFu, w.z >> 16, w.w & 0xFFFFu, w.w >> 16};
         uint32_t s = 0;
 #pragma unroll
@@ -294,13 +446,13 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
 #pragma unroll
         for (int i = 0; i < 8; ++i) { const uint32_t t = c[i]; c[i] = ex; ex += t; }
         w.x = c[0] | (c[1] << 16); w.y = c[2] | (c[3] << 16); w.z = c[4] | (c[5] << 16); w.w = c[6] | (c[7] << 16);
-        reinterpret_cast<uint4*>(sm.cnt)[tid] = w;
+        reinterpret_cast<uint4*>(sm.cs)[tid] = w;
     }
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < kMItems; ++i) {
         const uint32_t e = tid + i * kMThreads;
-        if (e < count) sm.list[bucket_start(sm, bs[i] >> 16) + (bs[i] & 0xFFFFu)] = (uint16_t)e;
+        if (e < count) list16[bucket_start(sm, bs[i] >> 16) + (bs[i] & 0xFFFFu)] = (uint16_t)e;
     }
     __syncthreads();
     // exact rank inside the bucket: order by (key, element id) = (time, input order)
@@ -315,18 +467,18 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
             if (s1 - s0 > 1) {
                 const uint64_t key = tile_key(sm, e);
                 for (uint32_t m = s0; m < s1; ++m) {
-                    const uint32_t o = sm.list[m];
+                    const uint32_t o = list16[m];
                     const uint64_t ko = tile_key(sm, o);
                     r += (ko < key || (ko == key && o < e)) ? 1u : 0u;
                 }
             }
-            sm.inv[r] = (uint16_t)e;
+            inv16[r] = (uint16_t)e;
         }
     }
     __syncthreads();
     // coalesced output
     for (uint32_t r = tid; r < count; r += kMThreads) {
-        const uint32_t e = sm.inv[r];
+        const uint32_t e = inv16[r];
         out[out_base + r] = sm.tile[e];
         if (kPerm) {
             uint32_t lo = 0, hi = K;  // piece j with segstart[j] <= e < segstart[j+1]
@@ -337,6 +489,20 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
     }
     __syncthreads();
     return count;
+}
+
+// 32-bit keys when the chunk spans < 2^32 key units (block-uniform), else the general 64-bit path
+template <bool kPerm>
+__device__ __forceinline__ uint32_t sort_any(MergeSmem& sm, const uint4* __restrict__ in, uint4* __restrict__ out, uint32_t K,
+                                             const uint32_t* chunk_end, uint64_t Ta, uint64_t width, uint32_t out_base,
+                                             const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out,
+                                             bool check_runs, const uint32_t* __restrict__ run_begin,
+                                             int32_t* __restrict__ status, uint32_t& phase) {
+    if (width <= 0xFFFFFFFFull)
+        return sort_chunk32<kPerm>(sm, in, out, K, chunk_end, Ta, (uint32_t)width, out_base, perm_in, perm_out, check_runs,
+                                   run_begin, status, phase);
+    return sort_chunk<kPerm>(sm, in, out, K, chunk_end, Ta, width, out_base, perm_in, perm_out, check_runs, run_begin, status,
+                             phase);
 }
 
 template <bool kPerm>
@@ -375,7 +541,7 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     (void)nt;
     if (remaining <= (uint32_t)kCap) {  // the common case: the whole tile in one chunk
         if (remaining)
-            sort_chunk<kPerm>(sm, in, out, K, sm.end, Ta, DT, out_base, perm_in, perm_out, check_runs != 0, run_begin, status, phase);
+            sort_any<kPerm>(sm, in, out, K, sm.end, Ta, DT, out_base, perm_in, perm_out, check_runs != 0, run_begin, status, phase);
         return;
     }
     // ---- overflow sweep: chunks of <= kCap hits in key order ------------------------------------------
@@ -398,7 +564,7 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
         }
         __syncthreads();
         if (remaining <= (uint32_t)kCap) {
-            const uint32_t c = sort_chunk<kPerm>(sm, in, out, K, sm.end, kmin, kmax - kmin + 1 ? kmax - kmin + 1 : ~0ull,
+            const uint32_t c = sort_any<kPerm>(sm, in, out, K, sm.end, kmin, kmax - kmin + 1 ? kmax - kmin + 1 : ~0ull,
                                                  out_base, perm_in, perm_out, check_runs != 0, run_begin, status, phase);
             out_base += c;
             break;
@@ -438,7 +604,7 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
         uint32_t total;
         const uint32_t ex = block_exclusive_scan(c, sm.scan, &total);
         if (have_lo && total) {
-            sort_chunk<kPerm>(sm, in, out, K, sm.mid, kmin, xlo - kmin + 1, out_base, perm_in, perm_out, check_runs != 0,
+            sort_any<kPerm>(sm, in, out, K, sm.mid, kmin, xlo - kmin + 1, out_base, perm_in, perm_out, check_runs != 0,
                               run_begin, status, phase);
         } else {
             // tie block: every hit has key == kmin; the stable order is the run-major concatenation

@@ -79,8 +79,7 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
         one_seg = seg_b >= ghi;
     }
     const int64_t t0 = hit_time(__ldg(hits + glo));
-    const uint64_t span = udiff(hit_time(__ldg(hits + (ghi - 1))), t0);
-    const bool fits32 = span < 0xFFFFFFFFull;  // every staged time is t0 + (a 32-bit offset)
+    bool wide = false;  // some staged time is not t0 + (a 32-bit offset): sparse data, or an earlier time of another segment
     uint8_t* s_fb = reinterpret_cast<uint8_t*>(s_f);
 #pragma unroll
     for (int k = 0; k < kL1Per + 2; ++k) {
@@ -88,7 +87,9 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
         uint32_t tr = 0xFFFFFFFFu, ky = 0xFFFFFFFFu, q = 0;
         if (e >= e_lo && e < e_hi) {
             const uint4 v = __ldg(hits + (g0 + e));
-            tr = (uint32_t)udiff(hit_time(v), t0);
+            const uint64_t d64 = udiff(hit_time(v), t0);
+            wide |= d64 >= 0xFFFFFFFFull;
+            tr = (uint32_t)d64;
             ky = v.z;
             q = (v.w & 0xFFFFu) >= q_thresh ? (uint32_t)TT_Q : 0u;
         }
@@ -97,7 +98,7 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
         if (k >= 1 && k <= kL1Per) s_fb[e - kL1Halo] = (uint8_t)q;
     }
     if (tid < kL1Pad) { s_t[kL1Stage + tid] = 0xFFFFFFFFu; s_k[kL1Stage + tid] = 0xFFFFFFFFu; }
-    __syncthreads();
+    const bool fits32 = !__syncthreads_or(wide);
     const uint32_t lc32 = lc > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)lc;
     if (fits32) {
         const uint32_t t_last = s_t[e_hi - 1];
@@ -262,34 +263,51 @@ __device__ __forceinline__ bool edge_tp(const tt_geometry_dev& g, uint64_t W, ui
 __device__ __forceinline__ uint64_t absdiff(int64_t a, int64_t b) { return a >= b ? udiff(a, b) : udiff(b, a); }
 
 // ---- fast path, pass 1: neighbour rows.  One thread per L1 hit x; the candidates (L1 hits of the same
-// segment within +-Weff) are staged in shared memory per tile of 256 hits.  Row of x: lo = index of
-// the first candidate, 128-bit mask of the causal neighbours relative to lo.  A hit with more than
-// 128 candidates ("wide") goes to the slow list instead.
+// segment within +-Weff) are staged in shared memory per tile of 256 hits.  Row of x: a bit mask of its causal
+// neighbours over the L1 list, in a frame of kRowWords 32-bit words that starts at the word-aligned list
+// index 32 f (so two rows are brought to a common frame by a word offset, no bit shifts).  Two phases per
+// hit: (1) which candidates sit on a tower that is connected to x's tower at all -- a byte table of the
+// tower pairs in shared memory, no global gather (cfg4: 27 % of the candidates survive); (2) the table
+// entry and the time test for the survivors only.  A hit with more than kRowSpan candidates ("wide") goes
+// to the slow list instead.
 constexpr int kRowTile = 256;
-constexpr int kRowStage = 1536;   // staged records per tile (tile + halos)
+constexpr int kRowStage = 1536;          // staged records per tile (tile + halos)
+constexpr int kRowSpan = 256;            // candidates a row can hold
+constexpr int kRowWords = 10;            // (31 + kRowSpan) / 32 + 1 = 9, padded to a 48-byte row
+constexpr int kPairBytesMax = 16384;     // tower-pair byte table in shared memory: n_tower <= 128
 constexpr uint32_t kWide = 0xFFFFFFFFu;
 
-struct Row {  // 32 bytes
-    uint64_t m0, m1;
-    uint32_t lo, deg;
-    uint32_t pad0, pad1;
+struct Row {  // 48 bytes
+    uint32_t w[kRowWords];
+    uint32_t f;    // frame: bit b of w[k] <=> L1 list index 32 (f + k) + b;  kWide = no row (slow list)
+    uint32_t deg;  // number of neighbours | (number of words in use) << 16
 };
 
 __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restrict__ l1, const uint32_t* __restrict__ m_ptr,
                                                            const uint32_t* __restrict__ seg_off, uint32_t n_seg,
                                                            uint32_t n, tt_geometry_dev g, uint64_t W, uint32_t N,
-                                                           uint32_t mode, uint8_t* __restrict__ flags,
+                                                           uint32_t mode, uint32_t pair_smem, uint8_t* __restrict__ flags,
                                                            uint8_t* __restrict__ l2bit, Row* __restrict__ rows,
                                                            uint32_t* __restrict__ slow_list, uint32_t* __restrict__ slow_cnt) {
     __shared__ int64_t s_t[kRowStage];
     __shared__ uint32_t s_idx[kRowStage];
     __shared__ uint32_t s_tp[kRowStage];
+    __shared__ uint32_t s_row[kRowWords][kRowTile];
     __shared__ uint32_t s_range[2];
+    extern __shared__ __align__(16) unsigned char s_pair[];  // [n_tower * n_tower] block id, 0xFF = unconnected
     const uint32_t m = *m_ptr;
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const bool any_edge = g.max_dt >= 0;
     const uint64_t Weff = any_edge ? ((uint64_t)g.max_dt < W ? (uint64_t)g.max_dt : W) : 0;
     const uint32_t ntiles = (m + kRowTile - 1) / kRowTile;
+    const uint32_t nt = g.n_tower;
+    if (pair_smem && blockIdx.x < ntiles) {
+        for (uint32_t i = tid; i < nt * nt; i += kRowTile) {
+            const int32_t bi = __ldg(g.pair_block + i);
+            s_pair[i] = bi < 0 ? (unsigned char)0xFF : (unsigned char)bi;
+        }
+    }
+    const int32_t blk_single = nt == 1 ? __ldg(g.pair_block) : -1;
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const uint32_t x0 = tile * kRowTile, x1 = min(m, x0 + kRowTile);
         // stage range: [lo(x0), hi(x1-1)) -- warp 0 scans backwards from x0, warp 1 forwards from x1-1
@@ -335,8 +353,7 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
         const uint32_t x = x0 + tid;
         if (x < x1) {
             bool wide = !staged;
-            Row row;
-            row.m0 = row.m1 = 0; row.lo = kWide; row.deg = 0; row.pad0 = row.pad1 = 0;
+            uint32_t deg = 0, f = kWide, words = 0;
             if (staged) {
                 const uint32_t xl = x - ylo, cnt = yhi - ylo;
                 const int64_t tx = s_t[xl];
@@ -354,32 +371,65 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
                 a = xl + 1; b = cnt;
                 while (a < b) { const uint32_t mid = (a + b) >> 1; if (s_idx[mid] < sb && udiff(s_t[mid], tx) <= Weff) a = mid + 1; else b = mid; }
                 const uint32_t hi = a;
-                if (hi - lo > 128) wide = true;
+                if (hi - lo > (uint32_t)kRowSpan) wide = true;
                 else {
-                    uint64_t m0 = 0, m1 = 0;
-                    if (any_edge && tpx != kBadTp) {
+                    f = (ylo + lo) >> 5;
+                    const uint32_t boff = (ylo + lo) & 31u;      // bit of candidate y: boff + (y - lo)
+                    words = (boff + (hi - lo) + 31u) >> 5;       // <= 9
+                    const bool live = any_edge && tpx != kBadTp && (nt > 1 || blk_single >= 0);
+                    const uint32_t prow = (tpx >> 16) * nt;
+                    // phase 1: candidates on connected towers
+                    {
+                        uint32_t cur = 0, k = 0, bit = boff;
                         for (uint32_t y = lo; y < hi; ++y) {
-                            if (y == xl) continue;
-                            const bool e = edge_tp(g, W, absdiff(tx, s_t[y]), tpx, s_tp[y]);
-                            const uint32_t k = y - lo;
-                            if (e) { if (k < 64) m0 |= 1ull << k; else m1 |= 1ull << (k - 64); }
+                            const uint32_t tpy = s_tp[y];
+                            bool c = live && y != xl && tpy != kBadTp;
+                            if (c && pair_smem) c = s_pair[prow + (tpy >> 16)] != 0xFF;
+                            cur |= (c ? 1u : 0u) << bit;
+                            if (++bit == 32u) { s_row[k++][tid] = cur; cur = 0; bit = 0; }
                         }
+                        if (bit) s_row[k][tid] = cur;
                     }
-                    row.m0 = m0; row.m1 = m1; row.lo = ylo + lo;
-                    row.deg = __popcll(m0) + __popcll(m1);
+                    // phase 2: the table entry and the time test for the survivors
+                    const uint32_t px = tpx & 0xFFFFu;
+                    for (uint32_t k = 0; k < words; ++k) {
+                        uint32_t wv = s_row[k][tid], out = 0;
+                        while (wv) {
+                            const uint32_t b2 = (uint32_t)__ffs(wv) - 1u;
+                            wv &= wv - 1u;
+                            const uint32_t y = lo + (32u * k + b2) - boff;
+                            const uint32_t tpy = s_tp[y];
+                            int32_t bi;
+                            if (nt == 1) bi = blk_single;
+                            else if (pair_smem) bi = s_pair[prow + (tpy >> 16)];
+                            else bi = __ldg(g.pair_block + prow + (tpy >> 16));
+                            if (bi < 0) continue;
+                            const int32_t lim = __ldg(g.blocks + ((size_t)(uint32_t)bi * g.ppt + px) * g.ppt + (tpy & 0xFFFFu));
+                            if (lim < 0) continue;
+                            const uint64_t l = (uint64_t)lim < W ? (uint64_t)lim : W;
+                            if (absdiff(tx, s_t[y]) <= l) out |= 1u << b2;
+                        }
+                        s_row[k][tid] = out;
+                        deg += __popc(out);
+                    }
                 }
             }
+            Row row;
+#pragma unroll
+            for (int k = 0; k < kRowWords; ++k) row.w[k] = (!wide && (uint32_t)k < words) ? s_row[k][tid] : 0u;
+            row.f = wide ? kWide : f;
+            row.deg = deg | (words << 16);
             rows[x] = row;
             if (wide) {
                 l2bit[x] = 0;
                 slow_list[atomicAdd(slow_cnt, 1u)] = x;
             } else {
-                const bool star = row.deg + 1 >= N;
+                const bool star = deg + 1 >= N;
                 const bool decided = mode == 1 || N <= 2 || !star;  // clique test needed only for star hits, N > 2
-                uint32_t f = 0;
-                if (star) f |= TT_L2STAR;
-                if (decided && star) f |= TT_L2;
-                if (f) flags[l1[x].idx] |= (uint8_t)f;
+                uint32_t fl = 0;
+                if (star) fl |= TT_L2STAR;
+                if (decided && star) fl |= TT_L2;
+                if (fl) flags[l1[x].idx] |= (uint8_t)fl;
                 l2bit[x] = (decided && star) ? 1 : 0;
             }
         }
@@ -387,61 +437,77 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
     }
 }
 
-// ---- fast path, pass 2: exact clique test on the rows (no table lookups).  One thread per star hit.
-struct M128 { uint64_t a, b; };
-__device__ __forceinline__ M128 m_and(M128 x, M128 y) { return {x.a & y.a, x.b & y.b}; }
-__device__ __forceinline__ int m_pop(M128 x) { return __popcll(x.a) + __popcll(x.b); }
-__device__ __forceinline__ M128 m_shl(M128 x, uint32_t s) {  // s < 128
-    if (s == 0) return x;
-    if (s >= 64) return {0ull, x.a << (s - 64)};
-    return {x.a << s, (x.b << s) | (x.a >> (64 - s))};
-}
-__device__ __forceinline__ M128 m_shr(M128 x, uint32_t s) {
-    if (s == 0) return x;
-    if (s >= 64) return {x.b >> (s - 64), 0ull};
-    return {(x.a >> s) | (x.b << (64 - s)), x.b >> s};
-}
+// ---- fast path, pass 2: exact clique test on the rows (no table lookups).  One thread per star hit; the
+// rows of a tile of hits and of everything their masks can name (+-(kRowSpan - 1) list positions) are
+// staged in shared memory, so a neighbour's row is a shared-memory read at a word offset.
+constexpr int kClqTile = 256;
+constexpr int kClqStage = kClqTile + 2 * (kRowSpan - 1);  // 766 rows, 36.8 KB
 
-__global__ void __launch_bounds__(128) l2_clique_kernel(const L1Rec* __restrict__ l1, const uint32_t* __restrict__ m_ptr,
-                                                        const Row* __restrict__ rows, uint32_t N, uint32_t mode,
-                                                        uint8_t* __restrict__ flags, uint8_t* __restrict__ l2bit,
-                                                        uint32_t* __restrict__ slow_list, uint32_t* __restrict__ slow_cnt) {
+__global__ void __launch_bounds__(kClqTile) l2_clique_kernel(const L1Rec* __restrict__ l1, const uint32_t* __restrict__ m_ptr,
+                                                             const Row* __restrict__ rows, uint32_t N, uint32_t mode,
+                                                             uint8_t* __restrict__ flags, uint8_t* __restrict__ l2bit,
+                                                             uint32_t* __restrict__ slow_list, uint32_t* __restrict__ slow_cnt) {
     if (mode != 0 || N <= 2) return;
+    __shared__ __align__(16) Row s_rows[kClqStage];
     const uint32_t m = *m_ptr;
+    const uint32_t tid = threadIdx.x;
     const int K = (int)N - 1;  // clique size wanted among the neighbours of x
-    for (uint32_t x = blockIdx.x * blockDim.x + threadIdx.x; x < m; x += gridDim.x * blockDim.x) {
-        const Row rx = rows[x];
-        if (rx.lo == kWide || rx.deg + 1 < N) continue;
-        const M128 nx = {rx.m0, rx.m1};
-        M128 cand[TT_MAX_MULTIPLICITY];
-        cand[0] = nx;
-        int d = 0;
-        bool found = false, punt = false;
-        while (true) {
-            const int rem = K - d;
-            if (rem == 0) { found = true; break; }
-            if (m_pop(cand[d]) < rem) {
-                if (d == 0) break;
-                --d;
-                continue;
+    const uint32_t ntiles = (m + kClqTile - 1) / kClqTile;
+    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const uint32_t x0 = tile * kClqTile, x1 = min(m, x0 + kClqTile);
+        const uint32_t base = x0 >= (uint32_t)(kRowSpan - 1) ? x0 - (kRowSpan - 1) : 0u;
+        const uint32_t top = min(m, x1 + (uint32_t)(kRowSpan - 1));
+        {   // rows [base, top) as 16-byte pieces, coalesced
+            const uint4* src = reinterpret_cast<const uint4*>(rows + base);
+            uint4* dst = reinterpret_cast<uint4*>(s_rows);
+            const uint32_t pieces = (top - base) * (uint32_t)(sizeof(Row) / 16);
+            for (uint32_t i = tid; i < pieces; i += kClqTile) dst[i] = src[i];
+        }
+        __syncthreads();
+        const uint32_t x = x0 + tid;
+        if (x < x1) {
+            const Row& rx = s_rows[x - base];
+            if (rx.f != kWide && (rx.deg & 0xFFFFu) + 1 >= N) {
+                uint32_t cand[TT_MAX_MULTIPLICITY][kRowWords];
+                const int nw = (int)(rx.deg >> 16);  // words of the frame that can hold a neighbour of x
+                for (int i = 0; i < nw; ++i) cand[0][i] = rx.w[i];
+                const uint32_t fx = rx.f;
+                int d = 0;
+                bool found = false, punt = false;
+                while (true) {
+                    const int rem = K - d;
+                    if (rem == 0) { found = true; break; }
+                    int pop = 0;
+                    for (int i = 0; i < nw; ++i) pop += __popc(cand[d][i]);
+                    if (pop < rem) {
+                        if (d == 0) break;
+                        --d;
+                        continue;
+                    }
+                    // lowest candidate v, remove it, descend with cand & adj(v)
+                    uint32_t v = 0;
+                    for (int i = 0; i < nw; ++i)
+                        if (cand[d][i]) { v = 32u * (uint32_t)i + (uint32_t)__ffs(cand[d][i]) - 1u; break; }
+                    cand[d][v >> 5] &= ~(1u << (v & 31u));
+                    const Row& rv = s_rows[32u * fx + v - base];
+                    if (rv.f == kWide) { punt = true; break; }
+                    const int off = (int)fx - (int)rv.f;  // word i of x's frame is word i + off of v's
+                    for (int i = 0; i < nw; ++i) {
+                        const int j = i + off;
+                        const uint32_t a = (j >= 0 && j < kRowWords) ? rv.w[j] : 0u;
+                        cand[d + 1][i] = cand[d][i] & a;
+                    }
+                    ++d;
+                }
+                if (punt) {
+                    slow_list[atomicAdd(slow_cnt, 1u)] = x;
+                } else if (found) {
+                    flags[l1[x].idx] |= (uint8_t)TT_L2;
+                    l2bit[x] = 1;
+                }
             }
-            // lowest candidate v (x frame), remove it, descend with cand & adj(v)
-            int v;
-            if (cand[d].a) { v = __ffsll((long long)cand[d].a) - 1; cand[d].a &= cand[d].a - 1; }
-            else { v = 64 + __ffsll((long long)cand[d].b) - 1; cand[d].b &= cand[d].b - 1; }
-            const Row rv = rows[rx.lo + (uint32_t)v];
-            if (rv.lo == kWide) { punt = true; break; }
-            M128 av = {rv.m0, rv.m1};
-            av = rv.lo >= rx.lo ? m_shl(av, rv.lo - rx.lo) : m_shr(av, rx.lo - rv.lo);  // |shift| < 128 (windows overlap)
-            cand[d + 1] = m_and(cand[d], av);
-            ++d;
         }
-        if (punt) {
-            slow_list[atomicAdd(slow_cnt, 1u)] = x;
-        } else if (found) {
-            flags[l1[x].idx] |= (uint8_t)TT_L2;
-            l2bit[x] = 1;
-        }
+        __syncthreads();
     }
 }
 
@@ -741,12 +807,14 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
                                                          g->dev.n_pmt, g->dev.ppt, d_status);
     prof_mark(s, "trig.l2_rows");
     TT_CUDA_OK(cudaMemsetAsync(plan.slow_cnt, 0, sizeof(uint32_t), s));
-    TT_K(l2_rows_kernel)<<<kSMs * 8, kRowTile, 0, s>>>(plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev,
-                                                      (uint64_t)p->l2_window_ps, p->l2_multiplicity, p->l2_mode, d_flags,
-                                                      plan.l2bit, plan.rows, plan.slow_list, plan.slow_cnt);
+    const uint32_t nt2 = g->dev.n_tower * g->dev.n_tower;
+    const uint32_t pair_smem = (g->dev.n_tower > 1 && nt2 <= (uint32_t)kPairBytesMax && g->dev.n_blocks <= 255u) ? 1u : 0u;
+    TT_K(l2_rows_kernel)<<<kSMs * 5, kRowTile, pair_smem ? ((nt2 + 15u) & ~15u) : 0, s>>>(
+        plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps, p->l2_multiplicity, p->l2_mode,
+        pair_smem, d_flags, plan.l2bit, plan.rows, plan.slow_list, plan.slow_cnt);
     prof_mark(s, "trig.l2_clique");
-    TT_K(l2_clique_kernel)<<<kSMs * 16, 128, 0, s>>>(plan.l1, plan.m_total, plan.rows, p->l2_multiplicity, p->l2_mode,
-                                                     d_flags, plan.l2bit, plan.slow_list, plan.slow_cnt);
+    TT_K(l2_clique_kernel)<<<kSMs * 6, kClqTile, 0, s>>>(plan.l1, plan.m_total, plan.rows, p->l2_multiplicity, p->l2_mode,
+                                                        d_flags, plan.l2bit, plan.slow_list, plan.slow_cnt);
     prof_mark(s, "trig.l2_wide");
     TT_K(l2_wide_kernel)<<<kSMs * 4, kL2Warps * 32, sizeof(WideSmem) * kL2Warps, s>>>(
         plan.l1, plan.m_total, plan.slow_list, plan.slow_cnt, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps,
