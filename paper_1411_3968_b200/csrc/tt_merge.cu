@@ -39,6 +39,7 @@ struct LevelDev {
     uint32_t* splits;        // split table
     uint32_t* roff_next;     // [G+1] run offsets of the next level (= group boundaries)
     uint32_t* tile_g;        // [tiles] group of every tile
+    uint32_t* tile_base;     // [tiles + G + 1] hits of the group before tile k (nt + 1 entries per group, zeroed, summed by atomics)
     uint32_t R, G, F;
 };
 
@@ -155,6 +156,7 @@ __global__ void __launch_bounds__(256) merge_partition_kernel(LevelDev lv, const
         res = a;
     }
     lv.splits[lv.sbase[g] + (size_t)k * K + j] = res;
+    if (res != lv.roff[r0 + j]) atomicAdd(&lv.tile_base[lv.tbase[g] + g + k], res - lv.roff[r0 + j]);
     if (j == 0 && k < nt) lv.tile_g[lv.tbase[g] + k] = g;
 }
 
@@ -223,13 +225,18 @@ __device__ __forceinline__ uint32_t bucket_start(const MergeSmem& sm, uint32_t b
 // one 32-bit composite per hit gives the stable order by a single unsigned compare.
 template <bool kPerm>
 __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, uint4* __restrict__ out, uint32_t K,
-                                 const uint32_t* chunk_end, uint64_t Ta, uint32_t width, uint32_t out_base,
+                                 const uint32_t* chunk_end, uint64_t Ta, uint32_t width, uint32_t out_base, uint32_t out_end,
                                  const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out, bool check_runs,
-                                 const uint32_t* __restrict__ run_begin, int32_t* __restrict__ status, uint32_t& phase) {
+                                 const uint32_t* __restrict__ run_begin, const uint64_t* prev_pre,
+                                 int32_t* __restrict__ status, uint32_t& phase) {
     const uint32_t tid = threadIdx.x, lane = tid & 31;
     uint32_t my_len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
     uint32_t total;
     const uint32_t my_s0 = block_exclusive_scan(my_len, sm.scan, &total);
+    if (total > (uint32_t)kCap) {  // the split table and the pieces disagree: only with unsorted runs
+        if (tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
+        return total;
+    }
     if (tid < K) sm.segstart[tid] = my_s0;
     if (tid == 0) {
         sm.segstart[K] = total;
@@ -249,7 +256,7 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
     if (check_runs && tid < (uint32_t)kCap / 32) sm.pstart[tid] = 0;
     uint64_t prev_key = 0;
     bool has_prev = false;
-    if (check_runs && my_len && sm.cur[tid] > run_begin[tid]) { prev_key = key_at(in, sm.cur[tid] - 1); has_prev = true; }
+    if (check_runs && my_len && sm.cur[tid] > run_begin[tid]) { prev_key = prev_pre ? *prev_pre : key_at(in, sm.cur[tid] - 1); has_prev = true; }
     __syncthreads();
     if (check_runs && my_len) atomicOr(&sm.pstart[my_s0 >> 5], 1u << (my_s0 & 31));
     mbar_wait(&sm.mbar, phase);
@@ -338,7 +345,15 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
             uint32_t r = s0;
             if (cb > 1u) {
                 const uint32_t c = (fb[i] & 0xFFFFF000u) | e;
-                for (uint32_t m = s0; m < s0 + cb; ++m) r += sm.list[m] < c ? 1u : 0u;
+                if (cb <= 8u) {  // independent loads, no loop-carried latency
+#pragma unroll
+                    for (uint32_t q = 0; q < 8u; ++q) {
+                        const uint32_t o = q < cb ? sm.list[s0 + q] : 0xFFFFFFFFu;
+                        r += o < c ? 1u : 0u;
+                    }
+                } else {
+                    for (uint32_t m = s0; m < s0 + cb; ++m) r += sm.list[m] < c ? 1u : 0u;
+                }
             }
             inv16[r] = (uint16_t)e;  // cs[] was last read before the barrier above
         }
@@ -348,7 +363,7 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
 #pragma unroll
     for (int i = 0; i < kMItems; ++i) {
         const uint32_t r = tid + i * kMThreads;
-        if (r < count) {
+        if (r < count && out_base + r < out_end) {
             const uint32_t e = inv16[r];
             out[out_base + r] = sm.tile[e];
             if (kPerm) {
@@ -368,9 +383,10 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
 // `phase` is the parity of the TMA barrier for this use (flips every call).
 template <bool kPerm>
 __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint4* __restrict__ out, uint32_t K,
-                               const uint32_t* chunk_end, uint64_t Ta, uint64_t width, uint32_t out_base,
+                               const uint32_t* chunk_end, uint64_t Ta, uint64_t width, uint32_t out_base, uint32_t out_end,
                                const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out, bool check_runs,
-                               const uint32_t* __restrict__ run_begin, int32_t* __restrict__ status, uint32_t& phase) {
+                               const uint32_t* __restrict__ run_begin, const uint64_t* prev_pre,
+                               int32_t* __restrict__ status, uint32_t& phase) {
     const uint32_t tid = threadIdx.x;
     // tile-local piece starts
     uint32_t my_len = 0, my_s0 = 0;
@@ -378,6 +394,10 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
         my_len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
         uint32_t total;
         my_s0 = block_exclusive_scan(my_len, sm.scan, &total);
+        if (total > (uint32_t)kCap) {  // the split table and the pieces disagree: only with unsorted runs
+            if (tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
+            return total;
+        }
         if (tid < K) sm.segstart[tid] = my_s0;
         if (tid == 0) {
             sm.segstart[K] = total;
@@ -396,7 +416,7 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
     if (check_runs && tid < (uint32_t)kCap / 32) sm.pstart[tid] = 0;
     uint64_t prev_key = 0;
     bool has_prev = false;
-    if (check_runs && my_len && sm.cur[tid] > run_begin[tid]) { prev_key = key_at(in, sm.cur[tid] - 1); has_prev = true; }
+    if (check_runs && my_len && sm.cur[tid] > run_begin[tid]) { prev_key = prev_pre ? *prev_pre : key_at(in, sm.cur[tid] - 1); has_prev = true; }
     __syncthreads();
     if (check_runs && my_len) atomicOr(&sm.pstart[my_s0 >> 5], 1u << (my_s0 & 31));
     mbar_wait(&sm.mbar, phase);
@@ -477,7 +497,7 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
     }
     __syncthreads();
     // coalesced output
-    for (uint32_t r = tid; r < count; r += kMThreads) {
+    for (uint32_t r = tid; r < count && out_base + r < out_end; r += kMThreads) {
         const uint32_t e = inv16[r];
         out[out_base + r] = sm.tile[e];
         if (kPerm) {
@@ -495,14 +515,15 @@ __device__ uint32_t sort_chunk(MergeSmem& sm, const uint4* __restrict__ in, uint
 template <bool kPerm>
 __device__ __forceinline__ uint32_t sort_any(MergeSmem& sm, const uint4* __restrict__ in, uint4* __restrict__ out, uint32_t K,
                                              const uint32_t* chunk_end, uint64_t Ta, uint64_t width, uint32_t out_base,
-                                             const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out,
-                                             bool check_runs, const uint32_t* __restrict__ run_begin,
+                                             uint32_t out_end, const uint32_t* __restrict__ perm_in,
+                                             uint32_t* __restrict__ perm_out, bool check_runs,
+                                             const uint32_t* __restrict__ run_begin, const uint64_t* prev_pre,
                                              int32_t* __restrict__ status, uint32_t& phase) {
     if (width <= 0xFFFFFFFFull)
-        return sort_chunk32<kPerm>(sm, in, out, K, chunk_end, Ta, (uint32_t)width, out_base, perm_in, perm_out, check_runs,
-                                   run_begin, status, phase);
-    return sort_chunk<kPerm>(sm, in, out, K, chunk_end, Ta, width, out_base, perm_in, perm_out, check_runs, run_begin, status,
-                             phase);
+        return sort_chunk32<kPerm>(sm, in, out, K, chunk_end, Ta, (uint32_t)width, out_base, out_end, perm_in, perm_out,
+                                   check_runs, run_begin, prev_pre, status, phase);
+    return sort_chunk<kPerm>(sm, in, out, K, chunk_end, Ta, width, out_base, out_end, perm_in, perm_out, check_runs, run_begin,
+                             prev_pre, status, phase);
 }
 
 template <bool kPerm>
@@ -522,26 +543,30 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     const uint32_t* row0 = lv.splits + lv.sbase[g] + (size_t)k * K;
     const uint32_t* row1 = row0 + K;
     const uint32_t* run_begin = lv.roff + r0;
-    uint32_t before = 0, len = 0;
+    uint64_t prev0 = 0;  // key of the hit before the piece of run tid (run check), fetched early
     if (tid < K) {
         const uint32_t a = row0[tid];
         uint32_t b = row1[tid];
         if (b < a) b = a;  // only with unsorted runs (flagged by the run check)
         sm.cur[tid] = a;
         sm.end[tid] = b;
-        before = a - run_begin[tid];
-        len = b - a;
+        if (check_runs && b > a && a > run_begin[tid]) prev0 = key_at(in, a - 1);
     }
-    uint32_t out_base = lv.roff[r0] + block_sum(before, sm.scan);
-    uint32_t remaining = block_sum(len, sm.scan);
+    // hits of the group before this tile / in it: summed by the partition kernel
+    const uint32_t tb0 = lv.tile_base[lv.tbase[g] + g + k];
+    uint32_t out_base = lv.roff[r0] + tb0;
+    uint32_t remaining = lv.tile_base[lv.tbase[g] + g + k + 1] - tb0;
+    const uint32_t out_end = lv.roff[r0 + K];  // end of the group's output range
     __syncthreads();
     const uint64_t T0 = lv.gT0[g], DT = lv.gDT[g];
     uint64_t Ta = T0 + (uint64_t)k * DT;
     if (Ta < T0) Ta = ~0ull;
     (void)nt;
+    if (remaining > (uint32_t)kCap) remaining = block_sum(tid < K ? sm.end[tid] - sm.cur[tid] : 0u, sm.scan);  // from the pieces
     if (remaining <= (uint32_t)kCap) {  // the common case: the whole tile in one chunk
         if (remaining)
-            sort_any<kPerm>(sm, in, out, K, sm.end, Ta, DT, out_base, perm_in, perm_out, check_runs != 0, run_begin, status, phase);
+            sort_any<kPerm>(sm, in, out, K, sm.end, Ta, DT, out_base, out_end, perm_in, perm_out, check_runs != 0, run_begin,
+                            &prev0, status, phase);
         return;
     }
     // ---- overflow sweep: chunks of <= kCap hits in key order ------------------------------------------
@@ -565,7 +590,8 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
         __syncthreads();
         if (remaining <= (uint32_t)kCap) {
             const uint32_t c = sort_any<kPerm>(sm, in, out, K, sm.end, kmin, kmax - kmin + 1 ? kmax - kmin + 1 : ~0ull,
-                                                 out_base, perm_in, perm_out, check_runs != 0, run_begin, status, phase);
+                                               out_base, out_end, perm_in, perm_out, check_runs != 0, run_begin, nullptr, status,
+                                               phase);
             out_base += c;
             break;
         }
@@ -604,8 +630,8 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
         uint32_t total;
         const uint32_t ex = block_exclusive_scan(c, sm.scan, &total);
         if (have_lo && total) {
-            sort_any<kPerm>(sm, in, out, K, sm.mid, kmin, xlo - kmin + 1, out_base, perm_in, perm_out, check_runs != 0,
-                              run_begin, status, phase);
+            sort_any<kPerm>(sm, in, out, K, sm.mid, kmin, xlo - kmin + 1, out_base, out_end, perm_in, perm_out, check_runs != 0,
+                            run_begin, nullptr, status, phase);
         } else {
             // tie block: every hit has key == kmin; the stable order is the run-major concatenation
             if (tid < K) sm.segstart[tid] = ex;
@@ -615,8 +641,10 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
                 uint32_t lo2 = 0, hi2 = K;
                 while (hi2 - lo2 > 1) { const uint32_t mid = (lo2 + hi2) >> 1; if (sm.segstart[mid] <= e) lo2 = mid; else hi2 = mid; }
                 const uint32_t src = sm.cur[lo2] + (e - sm.segstart[lo2]);
-                out[out_base + e] = __ldg(in + src);
-                if (kPerm) perm_out[out_base + e] = perm_in ? perm_in[src] : src;
+                if (out_base + e < out_end) {
+                    out[out_base + e] = __ldg(in + src);
+                    if (kPerm) perm_out[out_base + e] = perm_in ? perm_in[src] : src;
+                }
             }
             __syncthreads();
         }
@@ -712,6 +740,7 @@ static void carve(Arena& a, const std::vector<LevelHost>& levels, uint32_t n, bo
         d.splits = a.take<uint32_t>((size_t)L.split_entries + 1);
         d.roff_next = a.take<uint32_t>(L.G + 1);
         d.tile_g = a.take<uint32_t>((size_t)L.tiles + 1);
+        d.tile_base = a.take<uint32_t>((size_t)L.tiles + L.G + 1);
     }
     const size_t nlev = levels.size();
     w.tmp[0] = nlev > 1 ? a.take<uint4>(n) : nullptr;
@@ -757,6 +786,7 @@ int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_
         TT_K(merge_setup_kernel)<<<1, 1024, 0, s>>>(d, src, n);
         if (levels[l].split_entries) {
             prof_mark(s, l == 0 ? "sort.merge_partition0" : "sort.merge_partition1");
+            TT_CUDA_OK(cudaMemsetAsync(d.tile_base, 0, ((size_t)levels[l].tiles + levels[l].G + 1) * sizeof(uint32_t), s));
             TT_K(merge_partition_kernel)<<<div_up(levels[l].split_entries, 256), 256, 0, s>>>(d, src, levels[l].split_entries);
         }
         if (levels[l].tiles) {
