@@ -262,18 +262,23 @@ __device__ __forceinline__ bool edge_tp(const tt_geometry_dev& g, uint64_t W, ui
 }
 __device__ __forceinline__ uint64_t absdiff(int64_t a, int64_t b) { return a >= b ? udiff(a, b) : udiff(b, a); }
 
-// ---- fast path, pass 1: neighbour rows.  One thread per L1 hit x; the candidates (L1 hits of the same
-// segment within +-Weff) are staged in shared memory per tile of 256 hits.  Row of x: a bit mask of its causal
-// neighbours over the L1 list, in a frame of kRowWords 32-bit words that starts at the word-aligned list
-// index 32 f (so two rows are brought to a common frame by a word offset, no bit shifts).  Two phases per
-// hit: (1) which candidates sit on a tower that is connected to x's tower at all -- a byte table of the
-// tower pairs in shared memory, no global gather (cfg4: 27 % of the candidates survive); (2) the table
-// entry and the time test for the survivors only.  A hit with more than kRowSpan candidates ("wide") goes
-// to the slow list instead.
+// ---- fast path, pass 1: neighbour rows.  One CTA per tile of 256 L1 hits x; the candidates (L1 hits of the
+// same segment within +-Weff) are staged in shared memory.  Row of x: a bit mask of its causal neighbours over
+// the L1 list, in a frame of kRowWords 32-bit words that starts at the word-aligned list index 32 f (so two rows
+// are brought to a common frame by a word offset, no bit shifts).  Three steps per tile:
+//   (1) thread per x: window [lo, hi) by binary search; which candidates sit on a tower that is connected to
+//       x's tower at all (a byte table of the tower pairs in shared memory, no global gather; cfg4: 27 %
+//       survive).  A pair inside the tile is owned by its earlier hit, so it is tested once.
+//   (2) the surviving (x, y) pairs of the whole tile are written to a dense list;
+//   (3) thread per pair: table entry + time test, result bits OR-ed into the rows of both hits.
+// A hit with more than kRowSpan candidates ("wide") goes to the slow list instead.
 constexpr int kRowTile = 256;
-constexpr int kRowStage = 1536;          // staged records per tile (tile + halos)
 constexpr int kRowSpan = 256;            // candidates a row can hold
+constexpr int kRowHalo = kRowSpan;       // a window of <= kRowSpan hits never leaves [x - 255, x + 256]
+constexpr int kRowStage = kRowTile + 2 * kRowHalo;  // staged records per tile: always [x0 - 256, x0 + 512)
+constexpr int kRowPer = kRowStage / kRowTile;  // 3
 constexpr int kRowWords = 10;            // (31 + kRowSpan) / 32 + 1 = 9, padded to a 48-byte row
+constexpr int kPairList = 2048;          // pairs tested per round
 constexpr int kPairBytesMax = 16384;     // tower-pair byte table in shared memory: n_tower <= 128
 constexpr uint32_t kWide = 0xFFFFFFFFu;
 
@@ -283,20 +288,29 @@ struct Row {  // 48 bytes
     uint32_t deg;  // number of neighbours | (number of words in use) << 16
 };
 
+struct RowSmem {
+    int64_t t[kRowStage];
+    uint32_t idx[kRowStage];
+    uint32_t tp[kRowStage];
+    uint32_t cand[kRowWords][kRowTile];  // step 1: owned candidates on connected towers (x's frame)
+    uint32_t row[kRowWords][kRowTile];   // step 3: causal neighbours (x's frame)
+    uint32_t lo[kRowTile];               // window start (staged index); kWide = wide / not staged
+    uint32_t boff[kRowTile];             // bit of candidate y in x's frame: boff + (y - lo)
+    uint32_t list[kPairList];            // pair: (x - x0) << 16 | staged index of y
+    uint32_t scan[33];
+};
+
 __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restrict__ l1, const uint32_t* __restrict__ m_ptr,
                                                            const uint32_t* __restrict__ seg_off, uint32_t n_seg,
                                                            uint32_t n, tt_geometry_dev g, uint64_t W, uint32_t N,
                                                            uint32_t mode, uint32_t pair_smem, uint8_t* __restrict__ flags,
                                                            uint8_t* __restrict__ l2bit, Row* __restrict__ rows,
                                                            uint32_t* __restrict__ slow_list, uint32_t* __restrict__ slow_cnt) {
-    __shared__ int64_t s_t[kRowStage];
-    __shared__ uint32_t s_idx[kRowStage];
-    __shared__ uint32_t s_tp[kRowStage];
-    __shared__ uint32_t s_row[kRowWords][kRowTile];
-    __shared__ uint32_t s_range[2];
-    extern __shared__ __align__(16) unsigned char s_pair[];  // [n_tower * n_tower] block id, 0xFF = unconnected
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    RowSmem& sm = *reinterpret_cast<RowSmem*>(smem_raw);
+    unsigned char* s_pair = smem_raw + sizeof(RowSmem);  // [n_tower * n_tower] block id, 0xFF = unconnected
     const uint32_t m = *m_ptr;
-    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t tid = threadIdx.x;
     const bool any_edge = g.max_dt >= 0;
     const uint64_t Weff = any_edge ? ((uint64_t)g.max_dt < W ? (uint64_t)g.max_dt : W) : 0;
     const uint32_t ntiles = (m + kRowTile - 1) / kRowTile;
@@ -308,115 +322,141 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
         }
     }
     const int32_t blk_single = nt == 1 ? __ldg(g.pair_block) : -1;
+    // staged slot e of a tile <-> list index x0 - kRowHalo + e; slots outside [0, m) hold a record that is in no window
+    L1Rec pre[kRowPer];
+    auto fetch = [&](uint32_t tile) {
+        const uint32_t x0 = tile * kRowTile;
+#pragma unroll
+        for (int k = 0; k < kRowPer; ++k) {
+            const uint32_t e = tid + k * kRowTile;
+            const uint32_t y = x0 - (uint32_t)kRowHalo + e;  // wraps below 0: then y >= m
+            L1Rec r;
+            r.t = 0; r.idx = 0xFFFFFFFFu; r.tp = kBadTp;
+            if (y < m) r = l1[y];
+            pre[k] = r;
+        }
+    };
+    if (blockIdx.x < ntiles) fetch(blockIdx.x);
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
         const uint32_t x0 = tile * kRowTile, x1 = min(m, x0 + kRowTile);
-        // stage range: [lo(x0), hi(x1-1)) -- warp 0 scans backwards from x0, warp 1 forwards from x1-1
-        if (warp == 0) {
-            const L1Rec r0 = l1[x0];
-            uint32_t sa = 0;
-            if (n_seg > 1) sa = __ldg(seg_off + find_segment(seg_off, n_seg, r0.idx));
-            uint32_t lo = x0;
-            for (uint32_t base = x0; base > 0;) {
-                const bool valid = base > lane;
-                bool in = false;
-                if (valid) { const L1Rec ry = l1[base - 1 - lane]; in = ry.idx >= sa && udiff(r0.t, ry.t) <= Weff; }
-                const uint32_t ib = __ballot_sync(0xffffffffu, in);
-                lo = base - __popc(ib);  // `in` is monotone: a prefix of the lanes
-                if (ib != 0xffffffffu) break;
-                base -= 32;
-            }
-            if (lane == 0) s_range[0] = lo;
-        } else if (warp == 1) {
-            const L1Rec r1 = l1[x1 - 1];
-            uint32_t sb = n;
-            if (n_seg > 1) sb = __ldg(seg_off + find_segment(seg_off, n_seg, r1.idx) + 1);
-            uint32_t hi = x1;
-            for (uint32_t base = x1; base < m; base += 32) {
-                const uint32_t y = base + lane;
-                bool in = false;
-                if (y < m) { const L1Rec ry = l1[y]; in = ry.idx < sb && udiff(ry.t, r1.t) <= Weff; }
-                const uint32_t ib = __ballot_sync(0xffffffffu, in);
-                hi = base + __popc(ib);
-                if (ib != 0xffffffffu) break;
-            }
-            if (lane == 0) s_range[1] = hi;
+        const uint32_t ylo = x0 - (uint32_t)kRowHalo;          // list index of staged slot 0 (modulo 2^32)
+        const uint32_t e_lo = x0 >= (uint32_t)kRowHalo ? 0u : (uint32_t)kRowHalo - x0;  // first real slot
+        const uint32_t e_hi = min((uint32_t)kRowStage, m - ylo);                       // end of the real slots
+#pragma unroll
+        for (int k = 0; k < kRowPer; ++k) {
+            const uint32_t e = tid + k * kRowTile;
+            sm.t[e] = pre[k].t; sm.idx[e] = pre[k].idx; sm.tp[e] = pre[k].tp;
         }
         __syncthreads();
-        const uint32_t ylo = s_range[0], yhi = s_range[1];
-        const bool staged = yhi - ylo <= (uint32_t)kRowStage;
-        if (staged)
-            for (uint32_t y = ylo + tid; y < yhi; y += kRowTile) {
-                const L1Rec r = l1[y];
-                s_t[y - ylo] = r.t; s_idx[y - ylo] = r.idx; s_tp[y - ylo] = r.tp;
-            }
-        __syncthreads();
+        if (tile + gridDim.x < ntiles) fetch(tile + gridDim.x);  // in flight while this tile is worked on
+        const bool staged = true;
         const uint32_t x = x0 + tid;
+        const uint32_t xl = x - ylo;   // staged index of x
+        const uint32_t t0l = x0 - ylo, t1l = x1 - ylo;  // staged range of the tile
+        // ---- step 1a: windows ----------------------------------------------------------------------------
+        uint32_t lo = 0, hi = 0, f = kWide, boff = 0, words = 0;
+        bool wide = false;
         if (x < x1) {
-            bool wide = !staged;
-            uint32_t deg = 0, f = kWide, words = 0;
+            wide = !staged;
             if (staged) {
-                const uint32_t xl = x - ylo, cnt = yhi - ylo;
-                const int64_t tx = s_t[xl];
-                const uint32_t ix = s_idx[xl], tpx = s_tp[xl];
+                const uint32_t cnt = e_hi;
+                const int64_t tx = sm.t[xl];
                 uint32_t sa = 0, sb = n;
                 if (n_seg > 1) {
-                    const uint32_t s = find_segment(seg_off, n_seg, ix);
+                    const uint32_t s = find_segment(seg_off, n_seg, sm.idx[xl]);
                     sa = __ldg(seg_off + s); sb = __ldg(seg_off + s + 1);
                 }
                 // first y <= x with idx >= sa and tx - t_y <= Weff (monotone false..true on [0, xl])
-                uint32_t a = 0, b = xl;
-                while (a < b) { const uint32_t mid = (a + b) >> 1; if (s_idx[mid] >= sa && udiff(tx, s_t[mid]) <= Weff) b = mid; else a = mid + 1; }
-                const uint32_t lo = a;
+                uint32_t a = e_lo, b = xl;
+                while (a < b) { const uint32_t mid = (a + b) >> 1; if (sm.idx[mid] >= sa && udiff(tx, sm.t[mid]) <= Weff) b = mid; else a = mid + 1; }
+                lo = a;
                 // first y > x that is out (idx >= sb or t_y - tx > Weff): monotone true..false on (xl, cnt)
                 a = xl + 1; b = cnt;
-                while (a < b) { const uint32_t mid = (a + b) >> 1; if (s_idx[mid] < sb && udiff(s_t[mid], tx) <= Weff) a = mid + 1; else b = mid; }
-                const uint32_t hi = a;
+                while (a < b) { const uint32_t mid = (a + b) >> 1; if (sm.idx[mid] < sb && udiff(sm.t[mid], tx) <= Weff) a = mid + 1; else b = mid; }
+                hi = a;
                 if (hi - lo > (uint32_t)kRowSpan) wide = true;
                 else {
                     f = (ylo + lo) >> 5;
-                    const uint32_t boff = (ylo + lo) & 31u;      // bit of candidate y: boff + (y - lo)
-                    words = (boff + (hi - lo) + 31u) >> 5;       // <= 9
-                    const bool live = any_edge && tpx != kBadTp && (nt > 1 || blk_single >= 0);
-                    const uint32_t prow = (tpx >> 16) * nt;
-                    // phase 1: candidates on connected towers
-                    {
-                        uint32_t cur = 0, k = 0, bit = boff;
-                        for (uint32_t y = lo; y < hi; ++y) {
-                            const uint32_t tpy = s_tp[y];
-                            bool c = live && y != xl && tpy != kBadTp;
-                            if (c && pair_smem) c = s_pair[prow + (tpy >> 16)] != 0xFF;
-                            cur |= (c ? 1u : 0u) << bit;
-                            if (++bit == 32u) { s_row[k++][tid] = cur; cur = 0; bit = 0; }
-                        }
-                        if (bit) s_row[k][tid] = cur;
-                    }
-                    // phase 2: the table entry and the time test for the survivors
-                    const uint32_t px = tpx & 0xFFFFu;
-                    for (uint32_t k = 0; k < words; ++k) {
-                        uint32_t wv = s_row[k][tid], out = 0;
-                        while (wv) {
-                            const uint32_t b2 = (uint32_t)__ffs(wv) - 1u;
-                            wv &= wv - 1u;
-                            const uint32_t y = lo + (32u * k + b2) - boff;
-                            const uint32_t tpy = s_tp[y];
-                            int32_t bi;
-                            if (nt == 1) bi = blk_single;
-                            else if (pair_smem) bi = s_pair[prow + (tpy >> 16)];
-                            else bi = __ldg(g.pair_block + prow + (tpy >> 16));
-                            if (bi < 0) continue;
-                            const int32_t lim = __ldg(g.blocks + ((size_t)(uint32_t)bi * g.ppt + px) * g.ppt + (tpy & 0xFFFFu));
-                            if (lim < 0) continue;
-                            const uint64_t l = (uint64_t)lim < W ? (uint64_t)lim : W;
-                            if (absdiff(tx, s_t[y]) <= l) out |= 1u << b2;
-                        }
-                        s_row[k][tid] = out;
-                        deg += __popc(out);
+                    boff = (ylo + lo) & 31u;
+                    words = (boff + (hi - lo) + 31u) >> 5;  // <= 9
+                }
+            }
+        }
+        sm.lo[tid] = (x < x1 && !wide) ? lo : kWide;
+        sm.boff[tid] = boff;
+#pragma unroll
+        for (int k = 0; k < kRowWords; ++k) { sm.cand[k][tid] = 0; sm.row[k][tid] = 0; }
+        __syncthreads();
+        // ---- step 1b: owned candidates on connected towers -------------------------------------------------
+        uint32_t npair = 0;
+        const uint32_t tpx = (x < x1 && staged) ? sm.tp[xl] : kBadTp;
+        const uint32_t prow = (tpx >> 16) * nt;
+        if (x < x1 && !wide && any_edge && tpx != kBadTp && (nt > 1 || blk_single >= 0)) {
+            uint32_t cur = 0, k = 0, bit = boff;
+            for (uint32_t y = lo; y < hi; ++y) {
+                const uint32_t tpy = sm.tp[y];
+                // owner of the pair: the earlier hit if both are in the tile and have rows, else whoever has a row here
+                bool c = y > xl || y < t0l || sm.lo[y - t0l] == kWide;
+                c = c && y != xl && tpy != kBadTp;
+                if (c && pair_smem) c = s_pair[prow + (tpy >> 16)] != 0xFF;
+                cur |= (c ? 1u : 0u) << bit;
+                if (++bit == 32u) { sm.cand[k++][tid] = cur; npair += __popc(cur); cur = 0; bit = 0; }
+            }
+            if (bit) { sm.cand[k][tid] = cur; npair += __popc(cur); }
+        }
+        // ---- steps 2, 3: dense pair list, rounds of kPairList ------------------------------------------------
+        uint32_t total;
+        const uint32_t poff = block_exclusive_scan(npair, sm.scan, &total);
+        for (uint32_t r0 = 0; r0 < total; r0 += kPairList) {
+            if (npair && poff < r0 + kPairList && poff + npair > r0) {
+                uint32_t p = poff;
+                for (uint32_t k = 0; k < words; ++k) {
+                    uint32_t wv = sm.cand[k][tid];
+                    while (wv) {
+                        const uint32_t b2 = (uint32_t)__ffs(wv) - 1u;
+                        wv &= wv - 1u;
+                        if (p >= r0 && p < r0 + kPairList) sm.list[p - r0] = (tid << 16) | (lo + (32u * k + b2) - boff);
+                        ++p;
                     }
                 }
             }
+            __syncthreads();
+            const uint32_t np = min((uint32_t)kPairList, total - r0);
+            for (uint32_t p = tid; p < np; p += kRowTile) {
+                const uint32_t pr = sm.list[p];
+                const uint32_t xt = pr >> 16, y = pr & 0xFFFFu;  // tile index of x, staged index of y
+                const uint32_t xs = t0l + xt;
+                const uint32_t tpa = sm.tp[xs], tpb = sm.tp[y];
+                int32_t bi;
+                if (nt == 1) bi = blk_single;
+                else if (pair_smem) { const uint32_t v = s_pair[(tpa >> 16) * nt + (tpb >> 16)]; bi = v == 0xFF ? -1 : (int32_t)v; }
+                else bi = __ldg(g.pair_block + (tpa >> 16) * nt + (tpb >> 16));
+                if (bi < 0) continue;
+                const int32_t lim = __ldg(g.blocks + ((size_t)(uint32_t)bi * g.ppt + (tpa & 0xFFFFu)) * g.ppt + (tpb & 0xFFFFu));
+                if (lim < 0) continue;
+                const uint64_t l = (uint64_t)lim < W ? (uint64_t)lim : W;
+                if (absdiff(sm.t[xs], sm.t[y]) > l) continue;
+                const uint32_t bx = sm.boff[xt] + (y - sm.lo[xt]);
+                atomicOr(&sm.row[bx >> 5][xt], 1u << (bx & 31u));
+                if (y >= t0l && y < t1l) {  // the partner is in the tile: its row gets the mirrored bit
+                    const uint32_t yt = y - t0l, ylo2 = sm.lo[yt];
+                    if (ylo2 != kWide) {
+                        const uint32_t by = sm.boff[yt] + (xs - ylo2);
+                        atomicOr(&sm.row[by >> 5][yt], 1u << (by & 31u));
+                    }
+                }
+            }
+            __syncthreads();
+        }
+        // ---- rows out -------------------------------------------------------------------------------------
+        if (x < x1) {
+            uint32_t deg = 0;
             Row row;
 #pragma unroll
-            for (int k = 0; k < kRowWords; ++k) row.w[k] = (!wide && (uint32_t)k < words) ? s_row[k][tid] : 0u;
+            for (int k = 0; k < kRowWords; ++k) {
+                row.w[k] = wide ? 0u : sm.row[k][tid];
+                deg += __popc(row.w[k]);
+            }
             row.f = wide ? kWide : f;
             row.deg = deg | (words << 16);
             rows[x] = row;
@@ -429,7 +469,7 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
                 uint32_t fl = 0;
                 if (star) fl |= TT_L2STAR;
                 if (decided && star) fl |= TT_L2;
-                if (fl) flags[l1[x].idx] |= (uint8_t)fl;
+                if (fl) flags[sm.idx[xl]] |= (uint8_t)fl;
                 l2bit[x] = (decided && star) ? 1 : 0;
             }
         }
@@ -794,6 +834,8 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     if (!attr_done) {
         TT_CUDA_OK(cudaFuncSetAttribute(l2_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)(sizeof(WideSmem) * kL2Warps)));
+        TT_CUDA_OK(cudaFuncSetAttribute(l2_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        (int)(sizeof(RowSmem) + kPairBytesMax)));
         attr_done = true;
     }
     prof_mark(s, "trig.l1_flags");
@@ -809,7 +851,8 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     TT_CUDA_OK(cudaMemsetAsync(plan.slow_cnt, 0, sizeof(uint32_t), s));
     const uint32_t nt2 = g->dev.n_tower * g->dev.n_tower;
     const uint32_t pair_smem = (g->dev.n_tower > 1 && nt2 <= (uint32_t)kPairBytesMax && g->dev.n_blocks <= 255u) ? 1u : 0u;
-    TT_K(l2_rows_kernel)<<<kSMs * 5, kRowTile, pair_smem ? ((nt2 + 15u) & ~15u) : 0, s>>>(
+    const size_t rows_smem = sizeof(RowSmem) + (pair_smem ? ((nt2 + 15u) & ~15u) : 0);
+    TT_K(l2_rows_kernel)<<<kSMs * 4, kRowTile, rows_smem, s>>>(
         plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps, p->l2_multiplicity, p->l2_mode,
         pair_smem, d_flags, plan.l2bit, plan.rows, plan.slow_list, plan.slow_cnt);
     prof_mark(s, "trig.l2_clique");
