@@ -33,7 +33,7 @@ METRIC = "hits/s sorted+triggered on 1 B200 (ms per 200 ms slice) and % of HBM r
 ALG_BYTES_PIPELINE = 50  # sort 16 r + 16 w, trigger 16 r + ~2 w
 ALG_BYTES = {"sort": 32, "trig": 18, "ev": 2}
 # bounded oracle sample per config (time_scale, seg_scale): ~10-30 s of single-thread CPU work
-ORACLE_SAMPLE = {0: (1.0, 1.0), 1: (1.0, 1.0), 2: (0.5, 1.0), 3: (1.0, 16 / 64), 4: (0.3, 1.0)}
+ORACLE_SAMPLE = {0: (1.0, 1.0), 1: (1.0, 1.0), 2: (0.5, 1.0), 3: (1.0, 16 / 64), 4: (0.5, 1.0)}
 
 
 def peaks():
@@ -94,7 +94,7 @@ def make_workload(cfg: int, rank: int, scale: float):
     from paper_1411_3968_b200 import workload as W
 
     if scale == 1.0:
-        return W.make_config(cfg, seed_offset=rank)
+        return W.make_config(cfg, seed_offset=rank)  # = sharding.workload_seed_offset(rank, 0, world)
     return W.make_config(cfg, time_scale=scale, seed_offset=rank)
 
 
@@ -219,15 +219,9 @@ def run_ours(args):
     B.prof_enable(False)
     clocks = sampler.stop()
     ms_step = ms_total / args.steps
-    if dist is not None:
-        t = torch.tensor([ms_step], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_step = float(t.item())
-        tn = torch.tensor([n], device="cuda", dtype=torch.float64)
-        dist.all_reduce(tn, op=dist.ReduceOp.SUM)
-        n_total = int(tn.item())
-    else:
-        n_total = n
+    from paper_1411_3968_b200 import sharding
+
+    ms_step, n_total = sharding.reduce_timing(ms_step, n, "cuda")  # max over ranks, whole-job hits
     value = n_total / (ms_step * 1e-3)
 
     # ---- roofline of the dominant kernel (device time from the stage events of the timed steps) ----
@@ -254,7 +248,7 @@ def run_ours(args):
                 "traffic": traffic, "peak_source": peak_src, "alg_bytes_per_launch": alg / max(launches_dom, 1),
                 "launches_per_step": launches_dom, "kernel_ms_per_step": dur_ms,
                 "share_of_step": dur_ms / (ms_total / args.steps)}
-    pipe_ach = ALG_BYTES_PIPELINE * n / (ms_total / args.steps * 1e-3) / 1e9
+    pipe_ach = ALG_BYTES_PIPELINE * n / (ms_total / args.steps * 1e-3) / 1e9  # this rank
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
     e2e = None
@@ -287,10 +281,7 @@ def run_ours(args):
         for _ in range(k2):
             host_step()
         dt = (time.perf_counter() - t0) / k2
-        if dist is not None:
-            t = torch.tensor([dt], device="cuda", dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
+        dt, _ = sharding.reduce_timing(dt, n, "cuda")
         ns, ne = int(min(h_cnt[0], seed_cap)), int(min(h_cnt[1], event_cap))
         e2e = {"value": n_total / dt, "unit": "hits/s", "ms_per_step": 1e3 * dt,
                "h2d_bytes_per_step": int(16 * n + 4 * (seg.count + 1) + 4 * (runs.count + 1)),
