@@ -237,13 +237,13 @@ def run_ours(args):
         # a stage that runs several times per step (radix passes) still has to move the algorithmic bytes once
         dur_ms = per_stage[dom]
         ach = alg / (dur_ms * 1e-3) / 1e9
-        traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        traffic = None  # dram__bytes_read + write per launch from the committed ncu --set full summary
+        tp = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tp):
-            try:
-                traffic = json.load(open(tp)).get(f"cfg{args.config}", {}).get(dom)
-            except Exception:
-                traffic = None
+            for ln in open(tp).read().splitlines()[1:]:
+                f = ln.split(",")
+                if len(f) >= 3 and f[0] == f"cfg{args.config}" and f[1] == dom:
+                    traffic = float(f[2])
         roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": traffic, "peak_source": peak_src, "alg_bytes_per_launch": alg / max(launches_dom, 1),
                 "launches_per_step": launches_dom, "kernel_ms_per_step": dur_ms,
