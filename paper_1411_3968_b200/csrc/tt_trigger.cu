@@ -53,15 +53,26 @@ __device__ __forceinline__ bool lc_scan_global(const uint4* __restrict__ hits, i
 
 constexpr int kL1Pad = 64;  // readable slack behind the staged arrays (speculative key reads)
 
+struct L1Smem {
+    uint32_t f[kL1Tile / 4];
+    uint32_t t[kL1Stage + kL1Pad];
+    uint32_t k[kL1Stage + kL1Pad];
+    uint16_t fl[kL1Stage + kL1Pad];
+    uint32_t red[kL1Threads / 32];
+};
+
 __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __restrict__ hits, uint32_t n,
                                                              const uint32_t* __restrict__ seg_off, uint32_t n_seg,
                                                              uint64_t lc, uint32_t q_thresh,
                                                              uint8_t* __restrict__ flags,
                                                              uint32_t* __restrict__ tile_cnt) {
-    __shared__ uint32_t s_t[kL1Stage + kL1Pad];   // time relative to the first staged hit
-    __shared__ uint32_t s_k[kL1Stage + kL1Pad];   // floor << 16 | pmt
-    __shared__ __align__(16) uint32_t s_f[kL1Tile / 4];  // flag bytes of the in-tile hits
-    __shared__ uint32_t s_red[kL1Threads / 32];
+    extern __shared__ __align__(16) unsigned char l1_smem_raw[];
+    L1Smem& l1s = *reinterpret_cast<L1Smem*>(l1_smem_raw);
+    uint32_t* const s_t = l1s.t;     // time relative to the first staged hit
+    uint32_t* const s_k = l1s.k;     // floor << 16 | pmt
+    uint16_t* const s_fl = l1s.fl;   // floor alone: the scan's first test is one 16-bit compare
+    uint32_t* const s_f = l1s.f;     // flag bytes of the in-tile hits
+    uint32_t* const s_red = l1s.red;
     const uint32_t tid = threadIdx.x, lane = tid & 31;
     const uint32_t tb = blockIdx.x * (uint32_t)kL1Tile;                 // first in-tile hit
     const uint32_t te = min(n, tb + (uint32_t)kL1Tile);                 // end of the tile
@@ -95,9 +106,10 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
         }
         s_t[e] = tr;
         s_k[e] = ky;
+        s_fl[e] = (uint16_t)(ky >> 16);
         if (k >= 1 && k <= kL1Per) s_fb[e - kL1Halo] = (uint8_t)q;
     }
-    if (tid < kL1Pad) { s_t[kL1Stage + tid] = 0xFFFFFFFFu; s_k[kL1Stage + tid] = 0xFFFFFFFFu; }
+    if (tid < kL1Pad) { s_t[kL1Stage + tid] = 0xFFFFFFFFu; s_k[kL1Stage + tid] = 0xFFFFFFFFu; s_fl[kL1Stage + tid] = 0xFFFFu; }
     const bool fits32 = !__syncthreads_or(wide);
     const uint32_t lc32 = lc > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)lc;
     if (fits32) {
@@ -109,7 +121,7 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
             const uint32_t w0 = e - lane;                       // first slot of this warp's chunk
             if (w0 >= e_te) break;                              // warp-uniform
             const bool valid = e >= e_lo && e < e_te;
-            const uint32_t ti = s_t[e], ki = s_k[e];
+            const uint32_t ti = s_t[e], ki = s_k[e], fi = ki >> 16;
             uint32_t jmax = e_hi, sa = seg_a, sb = seg_b;
             if (!one_seg && valid) {
                 const uint32_t s = find_segment(seg_off, n_seg, g0 + e);
@@ -122,12 +134,14 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
             for (uint32_t d0 = 1; d0 < dmax; d0 += 4) {
                 // does any hit of the chunk still have offset d0 inside its window?
                 if (!__any_sync(0xffffffffu, valid && (s_t[e + d0] - ti <= lc32))) break;
-#pragma unroll
-                for (uint32_t q = 0; q < 4; ++q) {
-                    const uint32_t j = e + d0 + q;
-                    const uint32_t x = s_k[j] ^ ki;
-                    if (x - 1u < 0xFFFFu) {                     // same floor, other PMT: rare; now the exact tests
-                        if (valid && j < jmax && s_t[j] - ti <= lc32) {
+                // four offsets at once: a hit of the same floor is rare (cfg4: 18 neighbours, 1400 floors)
+                const uint32_t f0 = s_fl[e + d0], f1 = s_fl[e + d0 + 1], f2 = s_fl[e + d0 + 2], f3 = s_fl[e + d0 + 3];
+                if ((f0 == fi) | (f1 == fi) | (f2 == fi) | (f3 == fi)) {
+#pragma unroll 1
+                    for (uint32_t q = 0; q < 4; ++q) {          // now the exact tests
+                        const uint32_t j = e + d0 + q;
+                        const uint32_t x = s_k[j] ^ ki;
+                        if (x - 1u < 0xFFFFu && valid && j < jmax && s_t[j] - ti <= lc32) {  // same floor, other PMT
                             found = true;
                             if (j >= (uint32_t)kL1Halo && j < e_te)
                                 atomicOr(&s_f[(j - kL1Halo) >> 2], (uint32_t)TT_LC << (8 * ((j - kL1Halo) & 3)));
@@ -834,12 +848,13 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     if (!attr_done) {
         TT_CUDA_OK(cudaFuncSetAttribute(l2_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)(sizeof(WideSmem) * kL2Warps)));
+        TT_CUDA_OK(cudaFuncSetAttribute(l1_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(L1Smem)));
         TT_CUDA_OK(cudaFuncSetAttribute(l2_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                         (int)(sizeof(RowSmem) + kPairBytesMax)));
         attr_done = true;
     }
     prof_mark(s, "trig.l1_flags");
-    TT_K(l1_tile_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,
+    TT_K(l1_tile_kernel)<<<plan.nblk, kL1Threads, sizeof(L1Smem), s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,
                                                     (uint64_t)p->lc_window_ps, p->q_thresh, d_flags, plan.blk_cnt);
     prof_mark(s, "trig.l1_scan");
     int rc = exclusive_scan_u32(plan.blk_cnt, plan.blk_cnt, plan.nblk, plan.scan_scratch, plan.m_total, s);
