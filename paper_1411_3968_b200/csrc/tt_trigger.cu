@@ -292,7 +292,7 @@ constexpr int kRowHalo = kRowSpan;       // a window of <= kRowSpan hits never l
 constexpr int kRowStage = kRowTile + 2 * kRowHalo;  // staged records per tile: always [x0 - 256, x0 + 512)
 constexpr int kRowPer = kRowStage / kRowTile;  // 3
 constexpr int kRowWords = 10;            // (31 + kRowSpan) / 32 + 1 = 9, padded to a 48-byte row
-constexpr int kPairList = 2048;          // pairs tested per round
+constexpr int kPairList = 2 * 256 * 16;   // pair list of one round: 256 hits x 16 offsets x (later + before-tile) candidates
 constexpr int kPairBytesMax = 16384;     // tower-pair byte table in shared memory: n_tower <= 128
 constexpr uint32_t kWide = 0xFFFFFFFFu;
 
@@ -306,12 +306,12 @@ struct RowSmem {
     int64_t t[kRowStage];
     uint32_t idx[kRowStage];
     uint32_t tp[kRowStage];
-    uint32_t cand[kRowWords][kRowTile];  // step 1: owned candidates on connected towers (x's frame)
     uint32_t row[kRowWords][kRowTile];   // step 3: causal neighbours (x's frame)
     uint32_t lo[kRowTile];               // window start (staged index); kWide = wide / not staged
     uint32_t boff[kRowTile];             // bit of candidate y in x's frame: boff + (y - lo)
-    uint32_t list[kPairList];            // pair: (x - x0) << 16 | staged index of y
-    uint32_t scan[33];
+    uint16_t list[kPairList];            // pair of the current round: stream << 12 | (x - x0) << 4 | offset in the round
+    uint32_t npairs;
+    uint32_t next;                       // next tile of this CTA (dynamic schedule: dense tiles cost 10x)
 };
 
 __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restrict__ l1, const uint32_t* __restrict__ m_ptr,
@@ -351,7 +351,8 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
         }
     };
     if (blockIdx.x < ntiles) fetch(blockIdx.x);
-    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    uint32_t* const tile_ctr = slow_cnt + 1;  // zeroed with slow_cnt
+    for (uint32_t tile = blockIdx.x; tile < ntiles;) {
         const uint32_t x0 = tile * kRowTile, x1 = min(m, x0 + kRowTile);
         const uint32_t ylo = x0 - (uint32_t)kRowHalo;          // list index of staged slot 0 (modulo 2^32)
         const uint32_t e_lo = x0 >= (uint32_t)kRowHalo ? 0u : (uint32_t)kRowHalo - x0;  // first real slot
@@ -362,7 +363,7 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
             sm.t[e] = pre[k].t; sm.idx[e] = pre[k].idx; sm.tp[e] = pre[k].tp;
         }
         __syncthreads();
-        if (tile + gridDim.x < ntiles) fetch(tile + gridDim.x);  // in flight while this tile is worked on
+        if (tid == 0) sm.next = gridDim.x + atomicAdd(tile_ctr, 1u);
         const bool staged = true;
         const uint32_t x = x0 + tid;
         const uint32_t xl = x - ylo;   // staged index of x
@@ -399,64 +400,89 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
         sm.lo[tid] = (x < x1 && !wide) ? lo : kWide;
         sm.boff[tid] = boff;
 #pragma unroll
-        for (int k = 0; k < kRowWords; ++k) { sm.cand[k][tid] = 0; sm.row[k][tid] = 0; }
+        for (int k = 0; k < kRowWords; ++k) sm.row[k][tid] = 0;
         __syncthreads();
-        // ---- step 1b: owned candidates on connected towers -------------------------------------------------
-        uint32_t npair = 0;
+        const uint32_t next_tile = sm.next;
+        if (next_tile < ntiles) fetch(next_tile);  // in flight while this tile is worked on
+        // ---- steps 1b-3 in rounds of 16 list offsets: every warp walks its 32 hits in lockstep over the later
+        // candidates y = x + 1 + d (a pair inside the tile is owned by its earlier hit, with or without a row, so it
+        // is tested once) and over the candidates before the tile, y = lo + d; the ones on connected towers
+        // (cfg4: ~27 %) are appended to the tile's pair list with one shared-memory atomic per warp and step,
+        // then tested one thread per pair.  256 hits x 16 offsets always fit the list.
         const uint32_t tpx = (x < x1 && staged) ? sm.tp[xl] : kBadTp;
         const uint32_t prow = (tpx >> 16) * nt;
-        if (x < x1 && !wide && any_edge && tpx != kBadTp && (nt > 1 || blk_single >= 0)) {
-            uint32_t cur = 0, k = 0, bit = boff;
-            for (uint32_t y = lo; y < hi; ++y) {
-                const uint32_t tpy = sm.tp[y];
-                // owner of the pair: the earlier hit if both are in the tile and have rows, else whoever has a row here
-                bool c = y > xl || y < t0l || sm.lo[y - t0l] == kWide;
-                c = c && y != xl && tpy != kBadTp;
-                if (c && pair_smem) c = s_pair[prow + (tpy >> 16)] != 0xFF;
-                cur |= (c ? 1u : 0u) << bit;
-                if (++bit == 32u) { sm.cand[k++][tid] = cur; npair += __popc(cur); cur = 0; bit = 0; }
-            }
-            if (bit) { sm.cand[k][tid] = cur; npair += __popc(cur); }
-        }
-        // ---- steps 2, 3: dense pair list, rounds of kPairList ------------------------------------------------
-        uint32_t total;
-        const uint32_t poff = block_exclusive_scan(npair, sm.scan, &total);
-        for (uint32_t r0 = 0; r0 < total; r0 += kPairList) {
-            if (npair && poff < r0 + kPairList && poff + npair > r0) {
-                uint32_t p = poff;
-                for (uint32_t k = 0; k < words; ++k) {
-                    uint32_t wv = sm.cand[k][tid];
-                    while (wv) {
-                        const uint32_t b2 = (uint32_t)__ffs(wv) - 1u;
-                        wv &= wv - 1u;
-                        if (p >= r0 && p < r0 + kPairList) sm.list[p - r0] = (tid << 16) | (lo + (32u * k + b2) - boff);
-                        ++p;
-                    }
+        const bool emits = x < x1 && any_edge && tpx != kBadTp && (nt > 1 || blk_single >= 0);
+        const uint32_t fwd_end = emits ? (wide ? min(hi, t1l) : hi) : 0u;   // later candidates: [xl + 1, fwd_end)
+        const uint32_t back_end = (emits && !wide) ? min(xl, t0l) : 0u;      // candidates before the tile: [lo, back_end)
+        const uint32_t reach = max(fwd_end > xl + 1u ? fwd_end - xl - 1u : 0u, back_end > lo ? back_end - lo : 0u);
+        const uint32_t lane = tid & 31u;
+        for (uint32_t r = 0;; ++r) {
+            if (tid == 0) sm.npairs = 0;
+            if (!__syncthreads_or(reach > 16u * r)) break;
+            for (uint32_t dd = 0; dd < 16u; ++dd) {
+                const uint32_t d = 16u * r + dd;
+                const uint32_t yf = xl + 1u + d, yb = lo + d;
+                bool cf = yf < fwd_end, cb = yb < back_end;
+                if (!__any_sync(0xffffffffu, cf || cb)) break;  // offsets only grow
+                if (cf) {
+                    const uint32_t tpy = sm.tp[yf];
+                    cf = tpy != kBadTp && !(pair_smem && s_pair[prow + (tpy >> 16)] == 0xFF);
+                }
+                if (cb) {
+                    const uint32_t tpy = sm.tp[yb];
+                    cb = tpy != kBadTp && !(pair_smem && s_pair[prow + (tpy >> 16)] == 0xFF);
+                }
+                const uint32_t mf = __ballot_sync(0xffffffffu, cf), mb = __ballot_sync(0xffffffffu, cb);
+                const uint32_t cnt = (uint32_t)__popc(mf) + (uint32_t)__popc(mb);
+                if (cnt) {
+                    uint32_t base = 0;
+                    if (lane == 0) base = atomicAdd(&sm.npairs, cnt);
+                    base = __shfl_sync(0xffffffffu, base, 0);
+                    const uint32_t below = (1u << lane) - 1u;
+                    if (cf) sm.list[base + (uint32_t)__popc(mf & below)] = (uint16_t)((tid << 4) | dd);
+                    if (cb) sm.list[base + (uint32_t)__popc(mf) + (uint32_t)__popc(mb & below)] = (uint16_t)(0x1000u | (tid << 4) | dd);
                 }
             }
             __syncthreads();
-            const uint32_t np = min((uint32_t)kPairList, total - r0);
-            for (uint32_t p = tid; p < np; p += kRowTile) {
-                const uint32_t pr = sm.list[p];
-                const uint32_t xt = pr >> 16, y = pr & 0xFFFFu;  // tile index of x, staged index of y
-                const uint32_t xs = t0l + xt;
-                const uint32_t tpa = sm.tp[xs], tpb = sm.tp[y];
-                int32_t bi;
-                if (nt == 1) bi = blk_single;
-                else if (pair_smem) { const uint32_t v = s_pair[(tpa >> 16) * nt + (tpb >> 16)]; bi = v == 0xFF ? -1 : (int32_t)v; }
-                else bi = __ldg(g.pair_block + (tpa >> 16) * nt + (tpb >> 16));
-                if (bi < 0) continue;
-                const int32_t lim = __ldg(g.blocks + ((size_t)(uint32_t)bi * g.ppt + (tpa & 0xFFFFu)) * g.ppt + (tpb & 0xFFFFu));
-                if (lim < 0) continue;
-                const uint64_t l = (uint64_t)lim < W ? (uint64_t)lim : W;
-                if (absdiff(sm.t[xs], sm.t[y]) > l) continue;
-                const uint32_t bx = sm.boff[xt] + (y - sm.lo[xt]);
-                atomicOr(&sm.row[bx >> 5][xt], 1u << (bx & 31u));
-                if (y >= t0l && y < t1l) {  // the partner is in the tile: its row gets the mirrored bit
-                    const uint32_t yt = y - t0l, ylo2 = sm.lo[yt];
-                    if (ylo2 != kWide) {
-                        const uint32_t by = sm.boff[yt] + (xs - ylo2);
-                        atomicOr(&sm.row[by >> 5][yt], 1u << (by & 31u));
+            const uint32_t np = sm.npairs;  // <= 2 x 256 x 16 would overflow only if both streams were full: see kPairList
+            for (uint32_t p0 = tid; p0 < np; p0 += 4u * kRowTile) {  // four pairs per thread in flight: the table gather is the latency
+                uint32_t xt4[4], y4[4];
+                int32_t lim4[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const uint32_t p = p0 + (uint32_t)u * kRowTile;
+                    lim4[u] = -1; xt4[u] = 0; y4[u] = 0;
+                    if (p < np) {
+                        const uint32_t pr = sm.list[p];
+                        const uint32_t xt = (pr >> 4) & 0xFFu, xs = t0l + xt;  // tile index / staged index of x
+                        const uint32_t y = ((pr & 0x1000u) ? sm.lo[xt] : xs + 1u) + 16u * r + (pr & 15u);  // staged index of y
+                        const uint32_t tpa = sm.tp[xs], tpb = sm.tp[y];
+                        int32_t bi;
+                        if (nt == 1) bi = blk_single;
+                        else if (pair_smem) { const uint32_t v = s_pair[(tpa >> 16) * nt + (tpb >> 16)]; bi = v == 0xFF ? -1 : (int32_t)v; }
+                        else bi = __ldg(g.pair_block + (tpa >> 16) * nt + (tpb >> 16));
+                        xt4[u] = xt; y4[u] = y;
+                        if (bi >= 0) lim4[u] = __ldg(g.blocks + ((size_t)(uint32_t)bi * g.ppt + (tpa & 0xFFFFu)) * g.ppt + (tpb & 0xFFFFu));
+                    }
+                }
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    const int32_t lim = lim4[u];
+                    if (lim < 0) continue;
+                    const uint32_t xt = xt4[u], y = y4[u], xs = t0l + xt;
+                    const uint64_t l = (uint64_t)lim < W ? (uint64_t)lim : W;
+                    if (absdiff(sm.t[xs], sm.t[y]) > l) continue;
+                    const uint32_t xlo2 = sm.lo[xt];
+                    if (xlo2 != kWide) {
+                        const uint32_t bx = sm.boff[xt] + (y - xlo2);
+                        atomicOr(&sm.row[bx >> 5][xt], 1u << (bx & 31u));
+                    }
+                    if (y >= t0l && y < t1l) {  // the partner is in the tile: its row gets the mirrored bit
+                        const uint32_t yt = y - t0l, ylo2 = sm.lo[yt];
+                        if (ylo2 != kWide) {
+                            const uint32_t by = sm.boff[yt] + (xs - ylo2);
+                            atomicOr(&sm.row[by >> 5][yt], 1u << (by & 31u));
+                        }
                     }
                 }
             }
@@ -488,6 +514,7 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
             }
         }
         __syncthreads();
+        tile = next_tile;
     }
 }
 
@@ -507,10 +534,20 @@ __global__ void __launch_bounds__(kClqTile) l2_clique_kernel(const L1Rec* __rest
     const uint32_t tid = threadIdx.x;
     const int K = (int)N - 1;  // clique size wanted among the neighbours of x
     const uint32_t ntiles = (m + kClqTile - 1) / kClqTile;
-    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    __shared__ uint32_t s_next;
+    uint32_t* const tile_ctr = slow_cnt + 2;  // zeroed with slow_cnt
+    for (uint32_t tile = blockIdx.x; tile < ntiles;) {
+        if (tid == 0) s_next = gridDim.x + atomicAdd(tile_ctr, 1u);
         const uint32_t x0 = tile * kClqTile, x1 = min(m, x0 + kClqTile);
-        const uint32_t base = x0 >= (uint32_t)(kRowSpan - 1) ? x0 - (kRowSpan - 1) : 0u;
-        const uint32_t top = min(m, x1 + (uint32_t)(kRowSpan - 1));
+        // rows the masks of this tile can name: windows move forward with x, so the first and the last row of the
+        // tile bound them (a wide row at either end: the full +-(kRowSpan - 1))
+        uint32_t base = x0 >= (uint32_t)(kRowSpan - 1) ? x0 - (kRowSpan - 1) : 0u;
+        uint32_t top = min(m, x1 + (uint32_t)(kRowSpan - 1));
+        {
+            const uint32_t f0 = rows[x0].f, f1 = rows[x1 - 1].f, nw1 = rows[x1 - 1].deg >> 16;
+            if (f0 != kWide) base = max(base, min(x0, 32u * f0));
+            if (f1 != kWide) top = min(top, max(x1, 32u * (f1 + nw1)));
+        }
         {   // rows [base, top) as 16-byte pieces, coalesced
             const uint4* src = reinterpret_cast<const uint4*>(rows + base);
             uint4* dst = reinterpret_cast<uint4*>(s_rows);
@@ -526,14 +563,14 @@ __global__ void __launch_bounds__(kClqTile) l2_clique_kernel(const L1Rec* __rest
                 const int nw = (int)(rx.deg >> 16);  // words of the frame that can hold a neighbour of x
                 for (int i = 0; i < nw; ++i) cand[0][i] = rx.w[i];
                 const uint32_t fx = rx.f;
+                int cnt[TT_MAX_MULTIPLICITY + 1];  // candidates left on every level
+                cnt[0] = (int)(rx.deg & 0xFFFFu);
                 int d = 0;
                 bool found = false, punt = false;
                 while (true) {
                     const int rem = K - d;
                     if (rem == 0) { found = true; break; }
-                    int pop = 0;
-                    for (int i = 0; i < nw; ++i) pop += __popc(cand[d][i]);
-                    if (pop < rem) {
+                    if (cnt[d] < rem) {
                         if (d == 0) break;
                         --d;
                         continue;
@@ -543,15 +580,20 @@ __global__ void __launch_bounds__(kClqTile) l2_clique_kernel(const L1Rec* __rest
                     for (int i = 0; i < nw; ++i)
                         if (cand[d][i]) { v = 32u * (uint32_t)i + (uint32_t)__ffs(cand[d][i]) - 1u; break; }
                     cand[d][v >> 5] &= ~(1u << (v & 31u));
+                    cnt[d] -= 1;
+                    if (rem == 1) { found = true; break; }  // v completes the clique
                     const Row& rv = s_rows[32u * fx + v - base];
                     if (rv.f == kWide) { punt = true; break; }
                     const int off = (int)fx - (int)rv.f;  // word i of x's frame is word i + off of v's
+                    int c = 0;
                     for (int i = 0; i < nw; ++i) {
                         const int j = i + off;
                         const uint32_t a = (j >= 0 && j < kRowWords) ? rv.w[j] : 0u;
-                        cand[d + 1][i] = cand[d][i] & a;
+                        const uint32_t w = cand[d][i] & a;
+                        cand[d + 1][i] = w;
+                        c += __popc(w);
                     }
-                    ++d;
+                    if (c >= rem - 1) { cnt[d + 1] = c; ++d; }  // else no clique through v on this level
                 }
                 if (punt) {
                     slow_list[atomicAdd(slow_cnt, 1u)] = x;
@@ -561,7 +603,9 @@ __global__ void __launch_bounds__(kClqTile) l2_clique_kernel(const L1Rec* __rest
                 }
             }
         }
+        const uint32_t next_tile = s_next;  // written before the barrier after the staging
         __syncthreads();
+        tile = next_tile;
     }
 }
 
@@ -807,7 +851,7 @@ static void trigger_plan(Arena& a, uint32_t n, TriggerPlan& p) {
     p.l2bit = a.take<uint8_t>(n);
     p.rows = a.take<Row>(n);
     p.slow_list = a.take<uint32_t>(n);
-    p.slow_cnt = a.take<uint32_t>(1);
+    p.slow_cnt = a.take<uint32_t>(4);  // [0] slow-list length, [1] / [2] tile counters of the rows / clique kernels
 }
 
 }  // namespace tt
@@ -863,7 +907,7 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     TT_K(l1_compact_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1,
                                                          g->dev.n_pmt, g->dev.ppt, d_status);
     prof_mark(s, "trig.l2_rows");
-    TT_CUDA_OK(cudaMemsetAsync(plan.slow_cnt, 0, sizeof(uint32_t), s));
+    TT_CUDA_OK(cudaMemsetAsync(plan.slow_cnt, 0, 4 * sizeof(uint32_t), s));
     const uint32_t nt2 = g->dev.n_tower * g->dev.n_tower;
     const uint32_t pair_smem = (g->dev.n_tower > 1 && nt2 <= (uint32_t)kPairBytesMax && g->dev.n_blocks <= 255u) ? 1u : 0u;
     const size_t rows_smem = sizeof(RowSmem) + (pair_smem ? ((nt2 + 15u) & ~15u) : 0);
