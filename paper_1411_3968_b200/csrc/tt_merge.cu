@@ -38,7 +38,8 @@ struct LevelDev {
     uint64_t* gDT;           // [G] tile width in key units (>= 1)
     uint32_t* splits;        // split table
     uint32_t* roff_next;     // [G+1] run offsets of the next level (= group boundaries)
-    uint32_t* tile_g;        // [tiles] group of every tile
+    uint4* tile_desc;        // [tiles] {group, first run, runs K, tile k of the group}: one load instead of a chain
+    uint2* tile_desc2;       // [tiles] {split-table offset of the tile's row, tile_base index}
     uint32_t* tile_base;     // [tiles + G + 1] hits of the group before tile k (nt + 1 entries per group, zeroed, summed by atomics)
     uint32_t R, G, F;
 };
@@ -157,7 +158,10 @@ __global__ void __launch_bounds__(256) merge_partition_kernel(LevelDev lv, const
     }
     lv.splits[lv.sbase[g] + (size_t)k * K + j] = res;
     if (res != lv.roff[r0 + j]) atomicAdd(&lv.tile_base[lv.tbase[g] + g + k], res - lv.roff[r0 + j]);
-    if (j == 0 && k < nt) lv.tile_g[lv.tbase[g] + k] = g;
+    if (j == 0 && k < nt) {
+        lv.tile_desc[lv.tbase[g] + k] = make_uint4(g, r0, K, k);
+        lv.tile_desc2[lv.tbase[g] + k] = make_uint2(lv.sbase[g] + k * K, lv.tbase[g] + g + k);
+    }
 }
 
 // ---- the tile kernel ---------------------------------------------------------------------------------
@@ -537,10 +541,10 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     const uint32_t tid = threadIdx.x;
     if (tid == 0) mbar_init(&sm.mbar, 1);
     uint32_t phase = 0;
-    const uint32_t g = lv.tile_g[blockIdx.x], k = blockIdx.x - lv.tbase[g];
-    const uint32_t r0 = lv.gfirst[g], K = lv.gfirst[g + 1] - r0;
-    const uint32_t nt = lv.tbase[g + 1] - lv.tbase[g];
-    const uint32_t* row0 = lv.splits + lv.sbase[g] + (size_t)k * K;
+    const uint4 td = lv.tile_desc[blockIdx.x];
+    const uint2 td2 = lv.tile_desc2[blockIdx.x];
+    const uint32_t g = td.x, r0 = td.y, K = td.z, k = td.w;
+    const uint32_t* row0 = lv.splits + td2.x;
     const uint32_t* row1 = row0 + K;
     const uint32_t* run_begin = lv.roff + r0;
     uint64_t prev0 = 0;  // key of the hit before the piece of run tid (run check), fetched early
@@ -553,15 +557,14 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
         if (check_runs && b > a && a > run_begin[tid]) prev0 = key_at(in, a - 1);
     }
     // hits of the group before this tile / in it: summed by the partition kernel
-    const uint32_t tb0 = lv.tile_base[lv.tbase[g] + g + k];
+    const uint32_t tb0 = lv.tile_base[td2.y];
     uint32_t out_base = lv.roff[r0] + tb0;
-    uint32_t remaining = lv.tile_base[lv.tbase[g] + g + k + 1] - tb0;
+    uint32_t remaining = lv.tile_base[td2.y + 1] - tb0;
     const uint32_t out_end = lv.roff[r0 + K];  // end of the group's output range
     __syncthreads();
     const uint64_t T0 = lv.gT0[g], DT = lv.gDT[g];
     uint64_t Ta = T0 + (uint64_t)k * DT;
     if (Ta < T0) Ta = ~0ull;
-    (void)nt;
     if (remaining > (uint32_t)kCap) remaining = block_sum(tid < K ? sm.end[tid] - sm.cur[tid] : 0u, sm.scan);  // from the pieces
     if (remaining <= (uint32_t)kCap) {  // the common case: the whole tile in one chunk
         if (remaining)
@@ -739,7 +742,8 @@ static void carve(Arena& a, const std::vector<LevelHost>& levels, uint32_t n, bo
         d.gDT = a.take<uint64_t>(L.G + 1);
         d.splits = a.take<uint32_t>((size_t)L.split_entries + 1);
         d.roff_next = a.take<uint32_t>(L.G + 1);
-        d.tile_g = a.take<uint32_t>((size_t)L.tiles + 1);
+        d.tile_desc = a.take<uint4>((size_t)L.tiles + 1);
+        d.tile_desc2 = a.take<uint2>((size_t)L.tiles + 1);
         d.tile_base = a.take<uint32_t>((size_t)L.tiles + L.G + 1);
     }
     const size_t nlev = levels.size();
