@@ -222,6 +222,29 @@ __device__ __forceinline__ uint32_t bucket_start(const MergeSmem& sm, uint32_t b
     return (sm.cs[b >> 1] >> ((b & 1) * 16)) & 0xFFFFu;
 }
 
+// block-wide exclusive scan with ONE barrier (blockDim.x = kMThreads): warp scans, the warp totals through 16 words of
+// shared memory, and every warp scans those itself.  buf must not be rewritten before a later barrier.
+__device__ __forceinline__ uint32_t block_scan1(uint32_t v, uint32_t* buf, uint32_t* total) {
+    const uint32_t lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t inc = v;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(0xffffffffu, inc, d);
+        if (lane >= (uint32_t)d) inc += o;
+    }
+    if (lane == 31) buf[w] = inc;
+    __syncthreads();
+    const uint32_t s = lane < (uint32_t)(kMThreads / 32) ? buf[lane] : 0u;
+    uint32_t si = s;
+#pragma unroll
+    for (int d = 1; d < kMThreads / 32; d <<= 1) {
+        const uint32_t o = __shfl_up_sync(0xffffffffu, si, d);
+        if (lane >= (uint32_t)d) si += o;
+    }
+    *total = __shfl_sync(0xffffffffu, si, kMThreads / 32 - 1);
+    return __shfl_sync(0xffffffffu, si - s, w) + inc - v;
+}
+
 // ---- 32-bit-key chunk sort (the common case: the chunk spans < 2^32 ps) -----------------------------------
 // Same contract as sort_chunk below.  Counting sort on kCap fine buckets of the 32-bit key offset d = key - Ta:
 // bucket = hi32(d * scale), and the top 20 bits of lo32(d * scale) order the keys inside a bucket exactly
@@ -236,7 +259,7 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
     const uint32_t tid = threadIdx.x, lane = tid & 31;
     uint32_t my_len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
     uint32_t total;
-    const uint32_t my_s0 = block_exclusive_scan(my_len, sm.scan, &total);
+    const uint32_t my_s0 = block_scan1(my_len, sm.scan, &total);
     if (total > (uint32_t)kCap) {  // the split table and the pieces disagree: only with unsorted runs
         if (tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
         return total;
@@ -263,9 +286,9 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
     if (check_runs && my_len && sm.cur[tid] > run_begin[tid]) { prev_key = prev_pre ? *prev_pre : key_at(in, sm.cur[tid] - 1); has_prev = true; }
     __syncthreads();
     if (check_runs && my_len) atomicOr(&sm.pstart[my_s0 >> 5], 1u << (my_s0 & 31));
-    mbar_wait(&sm.mbar, phase);
+    mbar_wait(&sm.mbar, phase);  // every thread waits itself: the staged data is visible to it
     phase ^= 1u;
-    __syncthreads();
+    if (check_runs) __syncthreads();  // the piece-start bitmap
     const bool direct = width <= (uint32_t)kCap;
     const uint32_t scale = direct ? 0u : (uint32_t)(((uint64_t)kCap << 32) / width);
     const uint32_t Ta_lo = (uint32_t)Ta, Ta_hi = (uint32_t)(Ta >> 32);
@@ -322,7 +345,7 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
 #pragma unroll
         for (int i = 0; i < 8; ++i) sum += c[i];
         uint32_t tot;
-        uint32_t ex = block_exclusive_scan(sum, sm.scan, &tot);
+        uint32_t ex = block_scan1(sum, sm.scan + 16, &tot);
 #pragma unroll
         for (int i = 0; i < 8; ++i) { const uint32_t t = c[i]; c[i] = (ex << 16) | t; ex += t; }
         c4[2 * tid] = make_uint4(c[0], c[1], c[2], c[3]);
@@ -378,8 +401,7 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
             }
         }
     }
-    __syncthreads();
-    return count;
+    return count;  // the caller puts a barrier before the shared memory is used again
 }
 
 // Sort the chunk [cur_j, chunk_end_j) over the runs j < K (<= kCap hits in total) and write it at out_base.
@@ -635,6 +657,7 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
         if (have_lo && total) {
             sort_any<kPerm>(sm, in, out, K, sm.mid, kmin, xlo - kmin + 1, out_base, out_end, perm_in, perm_out, check_runs != 0,
                             run_begin, nullptr, status, phase);
+            __syncthreads();
         } else {
             // tie block: every hit has key == kmin; the stable order is the run-major concatenation
             if (tid < K) sm.segstart[tid] = ex;
