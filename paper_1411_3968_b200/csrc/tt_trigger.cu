@@ -57,7 +57,6 @@ struct L1Smem {
     uint32_t f[kL1Tile / 4];
     uint32_t t[kL1Stage + kL1Pad];
     uint32_t k[kL1Stage + kL1Pad];
-    uint16_t fl[kL1Stage + kL1Pad];
     uint32_t red[kL1Threads / 32];
 };
 
@@ -70,7 +69,6 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
     L1Smem& l1s = *reinterpret_cast<L1Smem*>(l1_smem_raw);
     uint32_t* const s_t = l1s.t;     // time relative to the first staged hit
     uint32_t* const s_k = l1s.k;     // floor << 16 | pmt
-    uint16_t* const s_fl = l1s.fl;   // floor alone: the scan's first test is one 16-bit compare
     uint32_t* const s_f = l1s.f;     // flag bytes of the in-tile hits
     uint32_t* const s_red = l1s.red;
     const uint32_t tid = threadIdx.x, lane = tid & 31;
@@ -106,10 +104,9 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
         }
         s_t[e] = tr;
         s_k[e] = ky;
-        s_fl[e] = (uint16_t)(ky >> 16);
         if (k >= 1 && k <= kL1Per) s_fb[e - kL1Halo] = (uint8_t)q;
     }
-    if (tid < kL1Pad) { s_t[kL1Stage + tid] = 0xFFFFFFFFu; s_k[kL1Stage + tid] = 0xFFFFFFFFu; s_fl[kL1Stage + tid] = 0xFFFFu; }
+    if (tid < kL1Pad) { s_t[kL1Stage + tid] = 0xFFFFFFFFu; s_k[kL1Stage + tid] = 0xFFFFFFFFu; }
     const bool fits32 = !__syncthreads_or(wide);
     const uint32_t lc32 = lc > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)lc;
     if (fits32) {
@@ -121,7 +118,7 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
             const uint32_t w0 = e - lane;                       // first slot of this warp's chunk
             if (w0 >= e_te) break;                              // warp-uniform
             const bool valid = e >= e_lo && e < e_te;
-            const uint32_t ti = s_t[e], ki = s_k[e], fi = ki >> 16;
+            const uint32_t ti = s_t[e], ki = s_k[e];
             uint32_t jmax = e_hi, sa = seg_a, sb = seg_b;
             if (!one_seg && valid) {
                 const uint32_t s = find_segment(seg_off, n_seg, g0 + e);
@@ -135,8 +132,8 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
                 // does any hit of the chunk still have offset d0 inside its window?
                 if (!__any_sync(0xffffffffu, valid && (s_t[e + d0] - ti <= lc32))) break;
                 // four offsets at once: a hit of the same floor is rare (cfg4: 18 neighbours, 1400 floors)
-                const uint32_t f0 = s_fl[e + d0], f1 = s_fl[e + d0 + 1], f2 = s_fl[e + d0 + 2], f3 = s_fl[e + d0 + 3];
-                if ((f0 == fi) | (f1 == fi) | (f2 == fi) | (f3 == fi)) {
+                const uint32_t x0 = s_k[e + d0] ^ ki, x1 = s_k[e + d0 + 1] ^ ki, x2 = s_k[e + d0 + 2] ^ ki, x3 = s_k[e + d0 + 3] ^ ki;
+                if ((x0 - 1u < 0xFFFFu) | (x1 - 1u < 0xFFFFu) | (x2 - 1u < 0xFFFFu) | (x3 - 1u < 0xFFFFu)) {  // same floor, other PMT
 #pragma unroll 1
                     for (uint32_t q = 0; q < 4; ++q) {          // now the exact tests
                         const uint32_t j = e + d0 + q;
