@@ -34,12 +34,17 @@ __device__ __forceinline__ bool is_head(const uint4* __restrict__ hits, const ui
 __global__ void __launch_bounds__(kEvThreads) ev_count_kernel(const uint4* __restrict__ hits,
                                                               const uint32_t* __restrict__ seeds,
                                                               const uint32_t* __restrict__ n_seeds_ptr, uint32_t seed_cap,
-                                                              SegCtx sc, uint64_t twoH, uint32_t* __restrict__ cnt) {
+                                                              SegCtx sc, uint64_t twoH, uint32_t* __restrict__ cnt,
+                                                              uint8_t* __restrict__ head) {
     const uint32_t ns = min(*n_seeds_ptr, seed_cap);
     uint32_t c0, c1;
     ev_chunk(ns, c0, c1);
     uint32_t c = 0;
-    for (uint32_t k = c0 + threadIdx.x; k < c1; k += kEvThreads) c += is_head(hits, seeds, k, sc, twoH) ? 1u : 0u;
+    for (uint32_t k = c0 + threadIdx.x; k < c1; k += kEvThreads) {  // the only pass that gathers the seed times
+        const bool h = is_head(hits, seeds, k, sc, twoH);
+        head[k] = h ? 1 : 0;
+        c += h ? 1u : 0u;
+    }
     __shared__ uint32_t sm[33];
     uint32_t total;
     block_exclusive_scan(c, sm, &total);
@@ -88,6 +93,7 @@ __global__ void __launch_bounds__(kEvThreads) ev_write_kernel(const uint4* __res
                                                               const uint32_t* __restrict__ n_seeds_ptr, uint32_t seed_cap,
                                                               SegCtx sc, uint64_t twoH, int64_t H,
                                                               const uint32_t* __restrict__ off,
+                                                              const uint8_t* __restrict__ head_flag,
                                                               tt_event* __restrict__ events, uint32_t event_cap) {
     __shared__ uint32_t sm[33];
     const uint32_t ns = min(*n_seeds_ptr, seed_cap);
@@ -97,31 +103,25 @@ __global__ void __launch_bounds__(kEvThreads) ev_write_kernel(const uint4* __res
     for (uint32_t base = c0; base < c1; base += kEvThreads) {
         const uint32_t k = base + threadIdx.x;
         const bool valid = k < c1;
-        const bool head = valid && is_head(hits, seeds, k, sc, twoH);
+        const bool head = valid && head_flag[k] != 0;
         uint32_t total;
         const uint32_t r = block_exclusive_scan(head ? 1u : 0u, sm, &total);
         if (valid) {
             const uint32_t e = run + r + (head ? 1u : 0u) - 1u;  // inclusive count - 1 (event 0 starts at seed 0)
-            const bool tail = (k + 1 == ns) || is_head(hits, seeds, k + 1, sc, twoH);
+            const bool tail = (k + 1 == ns) || head_flag[k + 1] != 0;
             if ((head || tail) && e < event_cap) {
                 const uint32_t i = seeds[k];
-                uint32_t sa = 0, sb = sc.n;
-                if (sc.n_seg > 1) {
-                    const uint32_t s = find_segment(sc.off, sc.n_seg, i);
-                    sa = __ldg(sc.off + s);
-                    sb = __ldg(sc.off + s + 1);
-                }
                 const int64_t t = hit_time(__ldg(hits + i));
+                // the hit ranges are searched by ev_fix_kernel (one thread per event, all in parallel): here only
+                // the seed's own hit index is left in hit_begin / hit_end
                 if (head) {
-                    const int64_t ts = (int64_t)((uint64_t)t - (uint64_t)H);
-                    events[e].t_start = ts;
-                    events[e].hit_begin = ts <= t ? lb_time(hits, sa, i, ts) : sa;  // wrapped below INT64_MIN: whole prefix
+                    events[e].t_start = (int64_t)((uint64_t)t - (uint64_t)H);
+                    events[e].hit_begin = i;
                     events[e].seed_begin = k;
                 }
                 if (tail) {
-                    const int64_t te = (int64_t)((uint64_t)t + (uint64_t)H);
-                    events[e].t_end = te;
-                    events[e].hit_end = te >= t ? ub_time(hits, i, sb, te) : sb;
+                    events[e].t_end = (int64_t)((uint64_t)t + (uint64_t)H);
+                    events[e].hit_end = i;
                     events[e].n_seeds = k + 1;  // end index; turned into a count by ev_fix_kernel
                 }
             }
@@ -130,11 +130,49 @@ __global__ void __launch_bounds__(kEvThreads) ev_write_kernel(const uint4* __res
     }
 }
 
-__global__ void __launch_bounds__(256) ev_fix_kernel(tt_event* __restrict__ events, const uint32_t* __restrict__ n_events_ptr,
+// one thread per event: seed count, and the hit range by galloping outwards from the first / last seed's hit
+// (the window is +-H around it: a few thousand hits, so the probes stay close together)
+__global__ void __launch_bounds__(256) ev_fix_kernel(const uint4* __restrict__ hits, SegCtx sc, int64_t H,
+                                                     tt_event* __restrict__ events, const uint32_t* __restrict__ n_events_ptr,
                                                      uint32_t event_cap) {
     const uint32_t ne = min(*n_events_ptr, event_cap);
-    for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += gridDim.x * blockDim.x)
-        events[e].n_seeds -= events[e].seed_begin;
+    for (uint32_t e = blockIdx.x * blockDim.x + threadIdx.x; e < ne; e += gridDim.x * blockDim.x) {
+        tt_event ev = events[e];
+        ev.n_seeds -= ev.seed_begin;
+        const uint32_t i0 = ev.hit_begin, i1 = ev.hit_end;  // hits of the first and of the last seed
+        uint32_t sa = 0, sb = sc.n;
+        if (sc.n_seg > 1) {
+            const uint32_t s = find_segment(sc.off, sc.n_seg, i0);
+            sa = __ldg(sc.off + s);
+            sb = __ldg(sc.off + s + 1);
+        }
+        const int64_t tf = (int64_t)((uint64_t)ev.t_start + (uint64_t)H), tl = (int64_t)((uint64_t)ev.t_end - (uint64_t)H);
+        if (ev.t_start <= tf) {  // first index of [sa, i0] with t >= t_start (t[i0] is one)
+            uint32_t hi = i0, lo, step = 32;
+            while (true) {
+                lo = hi - sa > step ? hi - step : sa;
+                if (lo == sa || hit_time(__ldg(hits + lo)) < ev.t_start) break;
+                hi = lo;
+                step <<= 1;
+            }
+            ev.hit_begin = lb_time(hits, lo, hi, ev.t_start);
+        } else {
+            ev.hit_begin = sa;  // wrapped below INT64_MIN: whole prefix
+        }
+        if (ev.t_end >= tl) {  // first index of (i1, sb) with t > t_end
+            uint32_t lo = i1 + 1, hi, step = 32;
+            while (true) {
+                hi = sb - lo > step ? lo + step : sb;
+                if (hi == sb || hit_time(__ldg(hits + (hi - 1))) > ev.t_end) break;
+                lo = hi;
+                step <<= 1;
+            }
+            ev.hit_end = ub_time(hits, lo, hi, ev.t_end);
+        } else {
+            ev.hit_end = sb;
+        }
+        events[e] = ev;
+    }
 }
 
 // ---- gather offsets: exclusive scan of event lengths (count on the device) ------------------------
@@ -199,24 +237,33 @@ __global__ void __launch_bounds__(kTagThreads) tag_gather_kernel(const uint4* __
     const uint32_t ne = min(*n_events_ptr, event_cap);
     if (ne == 0) return;
     const uint64_t i0l = ((uint64_t)blockIdx.x * kTagThreads + threadIdx.x) * kTagPer;
+    // first event with hit_end > i0: lane 0 of the warp searches for its index, the others walk on from there
+    uint32_t a = 0;
+    {
+        const uint64_t w0l = i0l - (uint64_t)(threadIdx.x & 31u) * kTagPer;  // first hit of the warp
+        if (w0l >= n) return;                                                // warp-uniform
+        if ((threadIdx.x & 31u) == 0) {
+            const uint32_t w0 = (uint32_t)w0l;
+            uint32_t b = ne;
+            while (a < b) {
+                const uint32_t mid = a + ((b - a) >> 1);
+                if (events[mid].hit_end <= w0) a = mid + 1; else b = mid;
+            }
+        }
+        a = __shfl_sync(0xffffffffu, a, 0);
+    }
     if (i0l >= n) return;
     const uint32_t i0 = (uint32_t)i0l;
     const uint32_t i1 = min(n, i0 + (uint32_t)kTagPer);
-    // first event with hit_end > i0
-    uint32_t a = 0, b = ne;
-    while (a < b) {
-        const uint32_t mid = a + ((b - a) >> 1);
-        if (events[mid].hit_end <= i0) a = mid + 1; else b = mid;
-    }
+    while (a < ne && events[a].hit_end <= i0) ++a;
     uint32_t mask = 0;
     for (uint32_t e = a; e < ne; ++e) {
         const uint32_t hb = events[e].hit_begin, he = events[e].hit_end;
         if (hb >= i1) break;
         const uint32_t lo = max(hb, i0), hi = min(he, i1);
-        for (uint32_t i = lo; i < hi; ++i) {
-            mask |= 1u << (i - i0);
-            if (gather) gather[goff[e] + (i - hb)] = __ldg(hits + i);
-        }
+        if (hi > lo) mask |= (0xFFFFFFFFu >> (32u - (hi - lo))) << (lo - i0);  // bits [lo - i0, hi - i0), at most 16
+        if (gather)
+            for (uint32_t i = lo; i < hi; ++i) gather[goff[e] + (i - hb)] = __ldg(hits + i);
     }
     if (flags && mask) {
         if (i1 - i0 == kTagPer && (((uintptr_t)(flags + i0)) & 15) == 0) {
@@ -237,12 +284,14 @@ __global__ void __launch_bounds__(kTagThreads) tag_gather_kernel(const uint4* __
 
 struct EventsPlan {
     uint32_t *cnt, *cnt2, *goff, *n_gathered_dummy;
+    uint8_t* head;  // [seed_cap] seed k opens an event
 };
-static void events_plan(Arena& a, uint32_t event_cap, bool gather, EventsPlan& p) {
+static void events_plan(Arena& a, uint32_t event_cap, uint32_t seed_cap, bool gather, EventsPlan& p) {
     p.cnt = a.take<uint32_t>(kEvBlocks);
     p.cnt2 = a.take<uint32_t>(kEvBlocks);
     p.n_gathered_dummy = a.take<uint32_t>(1);
     p.goff = a.take<uint32_t>(gather ? (size_t)event_cap : 1);
+    p.head = a.take<uint8_t>((size_t)seed_cap + 1);
 }
 
 }  // namespace tt
@@ -261,7 +310,7 @@ extern "C" int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint3
     if (h_seg_offsets[0] != 0 || h_seg_offsets[n_seg] != n) return TT_E_INVAL;
     Arena sizing(nullptr);
     EventsPlan plan;
-    events_plan(sizing, event_cap, true, plan);
+    events_plan(sizing, event_cap, seed_cap, true, plan);
     if (!d_ws) {
         *ws_bytes = sizing.off;
         return TT_OK;
@@ -273,7 +322,7 @@ extern "C" int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint3
     if (((uintptr_t)d_ws & 255) || ((uintptr_t)d_sorted & 15) || ((uintptr_t)d_gather & 15)) return TT_E_INVAL;
     cudaStream_t s = (cudaStream_t)stream;
     Arena a(d_ws);
-    events_plan(a, event_cap, true, plan);
+    events_plan(a, event_cap, seed_cap, true, plan);
     if (n == 0) {
         TT_CUDA_OK(cudaMemsetAsync(d_n_events, 0, sizeof(uint32_t), s));
         if (d_n_gathered) TT_CUDA_OK(cudaMemsetAsync(d_n_gathered, 0, sizeof(uint32_t), s));
@@ -283,11 +332,11 @@ extern "C" int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint3
     const uint64_t twoH = 2ull * (uint64_t)p->event_half_ps;
     const uint4* hits = (const uint4*)d_sorted;
     prof_mark(s, "ev.merge");
-    TT_K(ev_count_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(hits, d_seeds, d_n_seeds, seed_cap, sc, twoH, plan.cnt);
+    TT_K(ev_count_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(hits, d_seeds, d_n_seeds, seed_cap, sc, twoH, plan.cnt, plan.head);
     TT_K(ev_scan_kernel)<<<1, 1024, 0, s>>>(plan.cnt, kEvBlocks, d_n_events, event_cap, d_status);
     TT_K(ev_write_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(hits, d_seeds, d_n_seeds, seed_cap, sc, twoH, p->event_half_ps,
-                                                     plan.cnt, d_events, event_cap);
-    TT_K(ev_fix_kernel)<<<kSMs, 256, 0, s>>>(d_events, d_n_events, event_cap);
+                                                     plan.cnt, plan.head, d_events, event_cap);
+    TT_K(ev_fix_kernel)<<<kSMs, 256, 0, s>>>(hits, sc, p->event_half_ps, d_events, d_n_events, event_cap);
     if (d_gather || d_n_gathered) {
         prof_mark(s, "ev.gather_scan");
         TT_K(len_count_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(d_events, d_n_events, event_cap, plan.cnt2);
