@@ -153,6 +153,38 @@ __global__ void __launch_bounds__(256) merge_partition_kernel(LevelDev lv, const
         const uint64_t T0 = lv.gT0[g], DT = lv.gDT[g];
         const uint64_t add = (uint64_t)k * DT;  // k < 2^20, DT <= 2^64 / nt: no overflow of the product
         const uint64_t T = T0 + add < T0 ? ~0ull : T0 + add;
+        // Bisection down to a bracket of 128 hits (these probes are shared with the neighbouring boundaries and
+        // stay in the L2 cache), then ONE interpolated probe between the last keys seen below and above T and a
+        // short gallop: the bottom of the search touches 1-2 sectors of DRAM instead of ~5.  Exact for any data
+        // (only comparisons decide); the interpolation just picks the first probe.
+        uint64_t klo = 0, khi = 0;  // key[a - 1] < T and key[b] >= T once seen
+        bool have_lo = false, have_hi = false;
+        while (b - a > 128u) {
+            const uint32_t mid = a + ((b - a) >> 1);
+            const uint64_t km = key_at(hits, mid);
+            if (km < T) { a = mid + 1; klo = km; have_lo = true; } else { b = mid; khi = km; have_hi = true; }
+        }
+        if (have_lo && have_hi && b > a) {
+            // keys rise from klo at a - 1 to khi at b: first guess for the first index with key >= T
+            const float frac = (float)(T - klo) / (float)(khi - klo);  // in (0, 1]
+            uint32_t p = a + (uint32_t)(frac * (float)(b - a + 1));
+            p = p > a ? p - 1u : a;
+            if (p >= b) p = b - 1u;
+            uint32_t step = 2;
+            if (key_at(hits, p) < T) {  // answer in (p, b]
+                a = p + 1u;
+                while (a < b) {
+                    const uint32_t q = b - a > step ? a + step - 1u : b - 1u;
+                    if (key_at(hits, q) < T) { a = q + 1u; step <<= 1; } else { b = q; break; }
+                }
+            } else {                     // answer in [a, p]
+                b = p;
+                while (a < b) {
+                    const uint32_t q = b - a > step ? b - step : a;
+                    if (key_at(hits, q) >= T) { b = q; step <<= 1; } else { a = q + 1u; break; }
+                }
+            }
+        }
         while (a < b) { const uint32_t mid = a + ((b - a) >> 1); if (key_at(hits, mid) < T) a = mid + 1; else b = mid; }
         res = a;
     }
