@@ -298,3 +298,22 @@ def test_merge_path_edge_cases(kind, B, oracle_lib):
     assert st == 0
     assert out.tobytes() == srt.tobytes()
     assert (gperm == perm).all()
+
+
+def test_many_towers_global_pair_table(B, oracle_lib):
+    """More than 128 towers: the tower-pair byte table does not fit the L2 rows kernel's shared memory and the
+    pair-block ids are gathered from global memory instead (12 x 12 NEMO towers, 4608 PMTs, 8400-run style
+    two-level merge with 4608 runs)."""
+    geo = W.make_geometry("nemo", 12, 12)
+    assert geo.n_tower == 144
+    T_ps = 400_000_000  # 0.4 ms: ~100 k hits
+    h, rl, _ = W.make_segment(geo, np.full(geo.n_pmt, 55e3), 0, T_ps, 1, 6, seed=4242)
+    h["pad"] = (np.arange(len(h)) & 0xFFFF).astype(np.uint16)
+    seg = np.array([0, len(h)], dtype=np.uint32)
+    runs = np.zeros(len(rl) + 1, dtype=np.uint32)
+    np.cumsum(rl, out=runs[1:])
+    p = W.Params(l2_multiplicity=4)
+    o = oracle_chain(h, seg, geo, p)
+    r = B.process_slice(h, seg, runs, _geo(B, geo), _prm(B, p))
+    _compare(r, o)
+    assert r.status == 0 and len(o["seeds"]) > 0
