@@ -416,28 +416,26 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
         for (uint32_t r = 0;; ++r) {
             if (tid == 0) sm.npairs = 0;
             if (!__syncthreads_or(reach > 16u * r)) break;
-            for (uint32_t dd = 0; dd < 16u; ++dd) {
-                const uint32_t d = 16u * r + dd;
-                const uint32_t yf = xl + 1u + d, yb = lo + d;
-                bool cf = yf < fwd_end, cb = yb < back_end;
-                if (!__any_sync(0xffffffffu, cf || cb)) break;  // offsets only grow
-                if (cf) {
-                    const uint32_t tpy = sm.tp[yf];
-                    cf = tpy != kBadTp && !(pair_smem && s_pair[prow + (tpy >> 16)] == 0xFF);
-                }
-                if (cb) {
-                    const uint32_t tpy = sm.tp[yb];
-                    cb = tpy != kBadTp && !(pair_smem && s_pair[prow + (tpy >> 16)] == 0xFF);
-                }
-                const uint32_t mf = __ballot_sync(0xffffffffu, cf), mb = __ballot_sync(0xffffffffu, cb);
-                const uint32_t cnt = (uint32_t)__popc(mf) + (uint32_t)__popc(mb);
-                if (cnt) {
-                    uint32_t base = 0;
-                    if (lane == 0) base = atomicAdd(&sm.npairs, cnt);
-                    base = __shfl_sync(0xffffffffu, base, 0);
-                    const uint32_t below = (1u << lane) - 1u;
-                    if (cf) sm.list[base + (uint32_t)__popc(mf & below)] = (uint16_t)((tid << 4) | dd);
-                    if (cb) sm.list[base + (uint32_t)__popc(mf) + (uint32_t)__popc(mb & below)] = (uint16_t)(0x1000u | (tid << 4) | dd);
+            // one stream at a time: the candidates before the tile exist for the first hits of the tile only
+            // (most warps leave that loop at its first vote)
+#pragma unroll 1
+            for (uint32_t stream = 0; stream < 2u; ++stream) {
+                const uint32_t y0 = (stream ? lo : xl + 1u) + 16u * r, yend = stream ? back_end : fwd_end;
+                for (uint32_t dd = 0; dd < 16u; ++dd) {
+                    const uint32_t y = y0 + dd;
+                    bool c = y < yend;
+                    if (!__any_sync(0xffffffffu, c)) break;  // offsets only grow
+                    if (c) {
+                        const uint32_t tpy = sm.tp[y];
+                        c = tpy != kBadTp && !(pair_smem && s_pair[prow + (tpy >> 16)] == 0xFF);
+                    }
+                    const uint32_t mk = __ballot_sync(0xffffffffu, c);
+                    if (mk) {
+                        uint32_t base = 0;
+                        if (lane == 0) base = atomicAdd(&sm.npairs, (uint32_t)__popc(mk));
+                        base = __shfl_sync(0xffffffffu, base, 0);
+                        if (c) sm.list[base + (uint32_t)__popc(mk & ((1u << lane) - 1u))] = (uint16_t)((stream << 12) | (tid << 4) | dd);
+                    }
                 }
             }
             __syncthreads();
