@@ -304,8 +304,16 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
     fence_proxy_async();  // earlier generic-proxy accesses of the tile buffer are ordered before the bulk copies
     __syncthreads();
     const uint32_t count = total;
-    // stage the pieces: one TMA bulk copy per run piece, all in flight at once
-    if (my_len) bulk_g2s(&sm.tile[my_s0], in + sm.cur[tid], my_len * 16u, &sm.mbar);
+    // stage the pieces: one TMA bulk copy per run piece, all in flight at once.  Piece j is issued by lane j / 16
+    // of warp j % 16: a warp issues its lanes' copies one after the other, so the K copies are spread over all
+    // 16 warps instead of the first K / 32 (the others would wait for them at the next barrier).
+    {
+        const uint32_t jj = (tid & 31u) * (uint32_t)(kMThreads / 32) + (tid >> 5);
+        if (jj < K) {
+            const uint32_t s0 = sm.segstart[jj], len = sm.segstart[jj + 1] - s0;
+            if (len) bulk_g2s(&sm.tile[s0], in + sm.cur[jj], len * 16u, &sm.mbar);
+        }
+    }
     // meanwhile: clear the buckets and the piece-start bitmap, fetch the run predecessors
     {
         uint4* z = reinterpret_cast<uint4*>(sm.cs);
