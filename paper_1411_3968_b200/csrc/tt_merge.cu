@@ -287,7 +287,7 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
                                  const uint32_t* chunk_end, uint64_t Ta, uint32_t width, uint32_t out_base, uint32_t out_end,
                                  const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out, bool check_runs,
                                  const uint32_t* __restrict__ run_begin, const uint64_t* prev_pre,
-                                 int32_t* __restrict__ status, uint32_t& phase) {
+                                 int32_t* __restrict__ status, uint32_t& phase, bool cs_zeroed) {
     const uint32_t tid = threadIdx.x, lane = tid & 31;
     uint32_t my_len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
     uint32_t total;
@@ -314,8 +314,9 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
             if (len) bulk_g2s(&sm.tile[s0], in + sm.cur[jj], len * 16u, &sm.mbar);
         }
     }
-    // meanwhile: clear the buckets and the piece-start bitmap, fetch the run predecessors
-    {
+    // meanwhile: clear the buckets (unless the caller did, before an earlier barrier) and the piece-start bitmap,
+    // fetch the run predecessors
+    if (!cs_zeroed) {
         uint4* z = reinterpret_cast<uint4*>(sm.cs);
 #pragma unroll
         for (int i = 0; i < kCap / 4 / kMThreads; ++i) z[tid + i * kMThreads] = make_uint4(0, 0, 0, 0);
@@ -324,7 +325,7 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
     uint64_t prev_key = 0;
     bool has_prev = false;
     if (check_runs && my_len && sm.cur[tid] > run_begin[tid]) { prev_key = prev_pre ? *prev_pre : key_at(in, sm.cur[tid] - 1); has_prev = true; }
-    __syncthreads();
+    if (check_runs || !cs_zeroed) __syncthreads();
     if (check_runs && my_len) atomicOr(&sm.pstart[my_s0 >> 5], 1u << (my_s0 & 31));
     mbar_wait(&sm.mbar, phase);  // every thread waits itself: the staged data is visible to it
     phase ^= 1u;
@@ -584,10 +585,10 @@ __device__ __forceinline__ uint32_t sort_any(MergeSmem& sm, const uint4* __restr
                                              uint32_t out_end, const uint32_t* __restrict__ perm_in,
                                              uint32_t* __restrict__ perm_out, bool check_runs,
                                              const uint32_t* __restrict__ run_begin, const uint64_t* prev_pre,
-                                             int32_t* __restrict__ status, uint32_t& phase) {
+                                             int32_t* __restrict__ status, uint32_t& phase, bool cs_zeroed = false) {
     if (width <= 0xFFFFFFFFull)
         return sort_chunk32<kPerm>(sm, in, out, K, chunk_end, Ta, (uint32_t)width, out_base, out_end, perm_in, perm_out,
-                                   check_runs, run_begin, prev_pre, status, phase);
+                                   check_runs, run_begin, prev_pre, status, phase, cs_zeroed);
     return sort_chunk<kPerm>(sm, in, out, K, chunk_end, Ta, width, out_base, out_end, perm_in, perm_out, check_runs, run_begin,
                              prev_pre, status, phase);
 }
@@ -603,6 +604,11 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     const uint32_t tid = threadIdx.x;
     if (tid == 0) mbar_init(&sm.mbar, 1);
     uint32_t phase = 0;
+    {   // the bucket array is cleared while the tile's description is on its way; the barrier below orders it
+        uint4* z = reinterpret_cast<uint4*>(sm.cs);
+#pragma unroll
+        for (int i = 0; i < kCap / 4 / kMThreads; ++i) z[tid + i * kMThreads] = make_uint4(0, 0, 0, 0);
+    }
     const uint4 td = lv.tile_desc[blockIdx.x];
     const uint2 td2 = lv.tile_desc2[blockIdx.x];
     const uint32_t g = td.x, r0 = td.y, K = td.z, k = td.w;
@@ -631,7 +637,7 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     if (remaining <= (uint32_t)kCap) {  // the common case: the whole tile in one chunk
         if (remaining)
             sort_any<kPerm>(sm, in, out, K, sm.end, Ta, DT, out_base, out_end, perm_in, perm_out, check_runs != 0, run_begin,
-                            &prev0, status, phase);
+                            &prev0, status, phase, true);
         return;
     }
     // ---- overflow sweep: chunks of <= kCap hits in key order ------------------------------------------
