@@ -90,21 +90,35 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
     const int64_t t0 = hit_time(__ldg(hits + glo));
     bool wide = false;  // some staged time is not t0 + (a 32-bit offset): sparse data, or an earlier time of another segment
     uint8_t* s_fb = reinterpret_cast<uint8_t*>(s_f);
+    // batches of six unconditional loads (slots outside the staged range read the first staged hit and are
+    // discarded): all six are in flight before the first is used
+    constexpr int kBatch = 6;
+    static_assert((kL1Per + 2) % kBatch == 0, "staging batches");
 #pragma unroll
-    for (int k = 0; k < kL1Per + 2; ++k) {
-        const uint32_t e = tid + k * kL1Threads;
-        uint32_t tr = 0xFFFFFFFFu, ky = 0xFFFFFFFFu, q = 0;
-        if (e >= e_lo && e < e_hi) {
-            const uint4 v = __ldg(hits + (g0 + e));
-            const uint64_t d64 = udiff(hit_time(v), t0);
-            wide |= d64 >= 0xFFFFFFFFull;
-            tr = (uint32_t)d64;
-            ky = v.z;
-            q = (v.w & 0xFFFFu) >= q_thresh ? (uint32_t)TT_Q : 0u;
+    for (int k0 = 0; k0 < kL1Per + 2; k0 += kBatch) {
+        uint4 v[kBatch];
+#pragma unroll
+        for (int u = 0; u < kBatch; ++u) {
+            const uint32_t e = tid + (k0 + u) * kL1Threads;
+            const bool in = e >= e_lo && e < e_hi;
+            v[u] = __ldg(hits + (in ? g0 + e : glo));
         }
-        s_t[e] = tr;
-        s_k[e] = ky;
-        if (k >= 1 && k <= kL1Per) s_fb[e - kL1Halo] = (uint8_t)q;
+#pragma unroll
+        for (int u = 0; u < kBatch; ++u) {
+            const int k = k0 + u;
+            const uint32_t e = tid + k * kL1Threads;
+            uint32_t tr = 0xFFFFFFFFu, ky = 0xFFFFFFFFu, q = 0;
+            if (e >= e_lo && e < e_hi) {
+                const uint64_t d64 = udiff(hit_time(v[u]), t0);
+                wide |= d64 >= 0xFFFFFFFFull;
+                tr = (uint32_t)d64;
+                ky = v[u].z;
+                q = (v[u].w & 0xFFFFu) >= q_thresh ? (uint32_t)TT_Q : 0u;
+            }
+            s_t[e] = tr;
+            s_k[e] = ky;
+            if (k >= 1 && k <= kL1Per) s_fb[e - kL1Halo] = (uint8_t)q;
+        }
     }
     if (tid < kL1Pad) { s_t[kL1Stage + tid] = 0xFFFFFFFFu; s_k[kL1Stage + tid] = 0xFFFFFFFFu; }
     const bool fits32 = !__syncthreads_or(wide);
