@@ -148,14 +148,23 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
                 // four offsets at once: a hit of the same floor is rare (cfg4: 18 neighbours, 1400 floors)
                 const uint32_t x0 = s_k[e + d0] ^ ki, x1 = s_k[e + d0 + 1] ^ ki, x2 = s_k[e + d0 + 2] ^ ki, x3 = s_k[e + d0 + 3] ^ ki;
                 if ((x0 - 1u < 0xFFFFu) | (x1 - 1u < 0xFFFFu) | (x2 - 1u < 0xFFFFu) | (x3 - 1u < 0xFFFFu)) {  // same floor, other PMT
-#pragma unroll 1
-                    for (uint32_t q = 0; q < 4; ++q) {          // now the exact tests
-                        const uint32_t j = e + d0 + q;
-                        const uint32_t x = s_k[j] ^ ki;
-                        if (x - 1u < 0xFFFFu && valid && j < jmax && s_t[j] - ti <= lc32) {  // same floor, other PMT
-                            found = true;
-                            if (j >= (uint32_t)kL1Halo && j < e_te)
-                                atomicOr(&s_f[(j - kL1Halo) >> 2], (uint32_t)TT_LC << (8 * ((j - kL1Halo) & 3)));
+                    // the time tests, straight-line, before anything diverges: with few floors (one tower: 14) the
+                    // floor filter fires in almost every warp step, a real pair (floor AND window) stays rare
+                    const uint32_t j0 = e + d0;
+                    const bool m0 = (x0 - 1u < 0xFFFFu) && (s_t[j0] - ti <= lc32);
+                    const bool m1 = (x1 - 1u < 0xFFFFu) && (s_t[j0 + 1] - ti <= lc32);
+                    const bool m2 = (x2 - 1u < 0xFFFFu) && (s_t[j0 + 2] - ti <= lc32);
+                    const bool m3 = (x3 - 1u < 0xFFFFu) && (s_t[j0 + 3] - ti <= lc32);
+                    if (valid && (m0 | m1 | m2 | m3)) {
+                        const uint32_t mm = (m0 ? 1u : 0u) | (m1 ? 2u : 0u) | (m2 ? 4u : 0u) | (m3 ? 8u : 0u);
+#pragma unroll
+                        for (uint32_t q = 0; q < 4; ++q) {
+                            const uint32_t j = j0 + q;
+                            if (((mm >> q) & 1u) && j < jmax) {
+                                found = true;
+                                if (j >= (uint32_t)kL1Halo && j < e_te)
+                                    atomicOr(&s_f[(j - kL1Halo) >> 2], (uint32_t)TT_LC << (8 * ((j - kL1Halo) & 3)));
+                            }
                         }
                     }
                 }
