@@ -288,7 +288,7 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
                                  const uint32_t* __restrict__ perm_in, uint32_t* __restrict__ perm_out, bool check_runs,
                                  const uint32_t* __restrict__ run_begin, const uint64_t* prev_pre,
                                  int32_t* __restrict__ status, uint32_t& phase, bool cs_zeroed) {
-    const uint32_t tid = threadIdx.x, lane = tid & 31;
+    const uint32_t tid = threadIdx.x;
     uint32_t my_len = tid < K ? chunk_end[tid] - sm.cur[tid] : 0u;
     uint32_t total;
     const uint32_t my_s0 = block_scan1(my_len, sm.scan, &total);
@@ -343,24 +343,22 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
         fb[i] = 0; slot[i] = 0;
         uint32_t d = 0;
         bool oob = false;
+        uint2 kv = make_uint2(0u, 0u);
         if (e < count) {
             const uint2 v = *reinterpret_cast<const uint2*>(&sm.tile[e]);
+            kv = v;
             const uint32_t hi = (v.y ^ 0x80000000u) - Ta_hi - (v.x < Ta_lo ? 1u : 0u);  // high word of key - Ta
             d = v.x - Ta_lo;
             oob = hi != 0u || d >= width;          // only with unsorted runs (the splits assume sorted runs)
             if (oob) d = (hi & 0x80000000u) ? 0u : width - 1u;
         }
         if (check_runs) {
-            const uint32_t dp = __shfl_up_sync(0xffffffffu, d, 1);
+            // order inside a run piece: the staged predecessor's key, compared as (high, low) words -- the same for
+            // every lane (no shuffle, no lane-0 special case); piece starts are checked against prev_key above
             if (e < count && e > 0 && !((sm.pstart[e >> 5] >> (e & 31)) & 1u)) {
-                uint32_t pv = dp;
-                if (lane == 0) {  // predecessor held by another warp: recompute its offset
-                    const uint2 u = *reinterpret_cast<const uint2*>(&sm.tile[e - 1]);
-                    const uint32_t uh = (u.y ^ 0x80000000u) - Ta_hi - (u.x < Ta_lo ? 1u : 0u);
-                    pv = u.x - Ta_lo;
-                    if (uh != 0u || pv >= width) pv = (uh & 0x80000000u) ? 0u : width - 1u;
-                }
-                if (pv > d) unsorted = true;
+                const uint2 u = *reinterpret_cast<const uint2*>(&sm.tile[e - 1]);
+                const uint32_t uy = u.y ^ 0x80000000u, vy = kv.y ^ 0x80000000u;
+                if (uy > vy || (uy == vy && u.x > kv.x)) unsorted = true;
             }
             if (oob) unsorted = true;
         }
@@ -413,15 +411,14 @@ __device__ uint32_t sort_chunk32(MergeSmem& sm, const uint4* __restrict__ in, ui
             uint32_t r = s0;
             if (cb > 1u) {
                 const uint32_t c = (fb[i] & 0xFFFFF000u) | e;
-                if (cb <= 8u) {  // independent loads, no loop-carried latency
+                // four independent loads cover 99 % of the hits (bucket load 0.875: P(more than 4 in a bucket) = 1.2 %);
+                // the tail loop runs for the rare larger buckets only
 #pragma unroll
-                    for (uint32_t q = 0; q < 8u; ++q) {
-                        const uint32_t o = q < cb ? sm.list[s0 + q] : 0xFFFFFFFFu;
-                        r += o < c ? 1u : 0u;
-                    }
-                } else {
-                    for (uint32_t m = s0; m < s0 + cb; ++m) r += sm.list[m] < c ? 1u : 0u;
+                for (uint32_t q = 0; q < 4u; ++q) {
+                    const uint32_t o = q < cb ? sm.list[s0 + q] : 0xFFFFFFFFu;
+                    r += o < c ? 1u : 0u;
                 }
+                for (uint32_t q = 4u; q < cb; ++q) r += sm.list[s0 + q] < c ? 1u : 0u;
             }
             inv16[r] = (uint16_t)e;  // cs[] was last read before the barrier above
         }
@@ -629,8 +626,8 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     uint32_t out_base = lv.roff[r0] + tb0;
     uint32_t remaining = lv.tile_base[td2.y + 1] - tb0;
     const uint32_t out_end = lv.roff[r0 + K];  // end of the group's output range
+    const uint64_t T0 = lv.gT0[g], DT = lv.gDT[g];  // in flight together with the split rows, not after the barrier
     __syncthreads();
-    const uint64_t T0 = lv.gT0[g], DT = lv.gDT[g];
     uint64_t Ta = T0 + (uint64_t)k * DT;
     if (Ta < T0) Ta = ~0ull;
     if (remaining > (uint32_t)kCap) remaining = block_sum(tid < K ? sm.end[tid] - sm.cur[tid] : 0u, sm.scan);  // from the pieces
