@@ -330,7 +330,6 @@ struct RowSmem {
     uint32_t lo[kRowTile];               // window start (staged index); kWide = wide / not staged
     uint32_t boff[kRowTile];             // bit of candidate y in x's frame: boff + (y - lo)
     uint16_t list[kPairList];            // pair of the current round: stream << 12 | (x - x0) << 4 | offset in the round
-    uint32_t npairs;
     uint32_t next;                       // next tile of this CTA (dynamic schedule: dense tiles cost 10x)
 };
 
@@ -436,9 +435,13 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
         const uint32_t back_end = (emits && !wide) ? min(xl, t0l) : 0u;      // candidates before the tile: [lo, back_end)
         const uint32_t reach = max(fwd_end > xl + 1u ? fwd_end - xl - 1u : 0u, back_end > lo ? back_end - lo : 0u);
         const uint32_t lane = tid & 31u;
+        // Every warp keeps its own pair list (32 hits x 16 offsets x 2 streams = 1024 entries) and tests its own pairs:
+        // the rounds need no block-wide barrier and no shared counter (the row bits are OR-ed with atomics anyway), so
+        // a warp with a short reach does not wait for the dense ones round by round.
+        uint16_t* const wlist = sm.list + (tid >> 5) * (uint32_t)(kPairList / (kRowTile / 32));
         for (uint32_t r = 0;; ++r) {
-            if (tid == 0) sm.npairs = 0;
-            if (!__syncthreads_or(reach > 16u * r)) break;
+            if (!__any_sync(0xffffffffu, reach > 16u * r)) break;
+            uint32_t np = 0;  // warp-uniform
             // one stream at a time: the candidates before the tile exist for the first hits of the tile only
             // (most warps leave that loop at its first vote)
 #pragma unroll 1
@@ -453,25 +456,20 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
                         c = tpy != kBadTp && !(pair_smem && s_pair[prow + (tpy >> 16)] == 0xFF);
                     }
                     const uint32_t mk = __ballot_sync(0xffffffffu, c);
-                    if (mk) {
-                        uint32_t base = 0;
-                        if (lane == 0) base = atomicAdd(&sm.npairs, (uint32_t)__popc(mk));
-                        base = __shfl_sync(0xffffffffu, base, 0);
-                        if (c) sm.list[base + (uint32_t)__popc(mk & ((1u << lane) - 1u))] = (uint16_t)((stream << 12) | (tid << 4) | dd);
-                    }
+                    if (c) wlist[np + (uint32_t)__popc(mk & ((1u << lane) - 1u))] = (uint16_t)((stream << 12) | (tid << 4) | dd);
+                    np += (uint32_t)__popc(mk);
                 }
             }
-            __syncthreads();
-            const uint32_t np = sm.npairs;  // <= 2 x 256 x 16 would overflow only if both streams were full: see kPairList
-            for (uint32_t p0 = tid; p0 < np; p0 += 4u * kRowTile) {  // four pairs per thread in flight: the table gather is the latency
+            __syncwarp();
+            for (uint32_t p0 = lane; p0 < np; p0 += 4u * 32u) {  // four pairs per thread in flight: the table gather is the latency
                 uint32_t xt4[4], y4[4];
                 int32_t lim4[4];
 #pragma unroll
                 for (int u = 0; u < 4; ++u) {
-                    const uint32_t p = p0 + (uint32_t)u * kRowTile;
+                    const uint32_t p = p0 + (uint32_t)u * 32u;
                     lim4[u] = -1; xt4[u] = 0; y4[u] = 0;
                     if (p < np) {
-                        const uint32_t pr = sm.list[p];
+                        const uint32_t pr = wlist[p];
                         const uint32_t xt = (pr >> 4) & 0xFFu, xs = t0l + xt;  // tile index / staged index of x
                         const uint32_t y = ((pr & 0x1000u) ? sm.lo[xt] : xs + 1u) + 16u * r + (pr & 15u);  // staged index of y
                         const uint32_t tpa = sm.tp[xs], tpb = sm.tp[y];
@@ -504,8 +502,9 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
                     }
                 }
             }
-            __syncthreads();
+            __syncwarp();  // the list is rewritten in the next round
         }
+        __syncthreads();  // all rows complete (bits come from other warps too)
         // ---- rows out -------------------------------------------------------------------------------------
         if (x < x1) {
             uint32_t deg = 0;
