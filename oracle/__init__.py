@@ -114,3 +114,21 @@ def events(sorted_hits: np.ndarray, seg_offsets: np.ndarray, seeds: np.ndarray, 
     if rc != 0:
         raise ValueError("oracle_events: invalid parameters")
     return ev[: ne.value].copy()
+
+
+L0_START, L0_MEMBER = 1, 2
+
+
+def l0_ntw(sorted_hits: np.ndarray, seg_offsets: np.ndarray, *, multiplicity: int, window_ps: int):
+    """Level-0 N-in-TW trigger -> (l0 bytes [n], number of firing window starts)."""
+    h = np.ascontiguousarray(sorted_hits, dtype=HIT)
+    seg = np.ascontiguousarray(seg_offsets, dtype=np.uint32)
+    n = h.shape[0]
+    l0 = np.zeros(n, dtype=np.uint8)
+    ns = ctypes.c_uint32(0)
+    rc = lib().oracle_l0_ntw(_p(h), ctypes.c_uint32(n), _p(seg), ctypes.c_uint32(len(seg) - 1),
+                             ctypes.c_uint32(int(multiplicity)), ctypes.c_int64(int(window_ps)), _p(l0),
+                             ctypes.byref(ns))
+    if rc != 0:
+        raise ValueError("oracle_l0_ntw: invalid parameters")
+    return l0, ns.value

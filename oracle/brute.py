@@ -99,3 +99,28 @@ def event_groups(seed_t, seed_seg, H: int):
         out.append((int(seed_seg[members[0]]), min(ts) - H, max(ts) + H, sorted(members)))
     out.sort(key=lambda e: (e[0], e[1]))
     return out
+
+
+def l0_ntw(h: np.ndarray, seg_offsets, N: int, tw_ps: int) -> np.ndarray:
+    """PAPER.md:59 'looking for 7 hits in TW'.  Counting formulation on half-open time intervals, no k+N-1
+    indexing: hit k is a firing start <=> at least N hits of its segment with index >= k have t < t_k + TW;
+    hit i is a member <=> some hit a of its segment has t_a <= t_i < t_a + TW and at least N hits of the segment
+    lie in [t_a, t_a + TW)  (the hits of such an interval are consecutive in time order, so N consecutive ones
+    containing i span less than TW)."""
+    n = len(h)
+    sg = seg_id(n, seg_offsets)
+    t = [int(x) for x in h["t_ps"]]
+    out = np.zeros(n, dtype=np.uint8)
+    for k in range(n):
+        c = sum(1 for j in range(k, n) if sg[j] == sg[k] and t[j] < t[k] + tw_ps)
+        if tw_ps > 0 and c >= N:
+            out[k] |= 1
+    for i in range(n):
+        for a in range(n):
+            if sg[a] != sg[i] or not (t[a] <= t[i] < t[a] + tw_ps):
+                continue
+            c = sum(1 for j in range(n) if sg[j] == sg[a] and t[a] <= t[j] < t[a] + tw_ps)
+            if c >= N:
+                out[i] |= 2
+                break
+    return out

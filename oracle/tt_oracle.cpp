@@ -17,6 +17,10 @@
 //                   pairwise L2 condition of north_star / BASELINE.json configs[0].
 //   oracle_events   PAPER.md:23 ("a 6 us time window ... centered at the time of the trigger
 //                   seed"), PAPER.md:67 ("all hits within +-3 us are tagged").
+//   oracle_l0_ntw   PAPER.md:59 ("N7TW1000: looking for 7 hits in TW = 1000 ns:
+//                   hit[i].time-hit[i+7].time< TW"), PAPER.md:73 (N7TW500 for the 84-PMT tower)
+//                   (used first, "as level 0 trigger").  DESIGN.md reading R14: the printed formula has the
+//                   sign reversed and 7 hits span i..i+6, so the test is t[k+N-1] - t[k] < TW, strict as printed.
 //
 // Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force pair / subset enumeration written
 // separately in oracle/brute.py, numpy stable argsort, Poisson closed forms, N-in-TW special
@@ -204,6 +208,32 @@ int oracle_events(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n_
         }
     }
     *n_events = ne;
+    return 0;
+}
+
+// Level-0 N-in-TW trigger on time-sorted hits (reading R14).  Inside each segment, window
+// start k fires <=> hit k+N-1 exists in the segment and t[k+N-1] - t[k] < TW (strict).  l0[i] bit 0 (1) =
+// i is a firing window start; bit 1 (2) = i is one of the N hits k..k+N-1 of some firing window.
+// *n_start = number of firing starts.  N >= 1; TW <= 0 never fires.
+int oracle_l0_ntw(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n_seg, uint32_t N, int64_t TW,
+                  uint8_t* l0, uint32_t* n_start) {
+    if (N < 1) return -1;
+    for (uint32_t i = 0; i < n; ++i) l0[i] = 0;
+    uint32_t count = 0;
+    for (uint32_t s = 0; s < n_seg; ++s) {
+        const uint64_t a = seg_off[s], b = seg_off[s + 1];
+        for (uint64_t k = a; k < b; ++k) {
+            const uint64_t last = k + (uint64_t)N - 1;
+            if (last >= b) break;  // fewer than N hits left in the segment
+            const __int128 dt = (__int128)h[last].t_ps - (__int128)h[k].t_ps;
+            if (dt < (__int128)TW) {
+                l0[k] |= 1;
+                for (uint64_t j = k; j <= last; ++j) l0[j] |= 2;
+                ++count;
+            }
+        }
+    }
+    *n_start = count;
     return 0;
 }
 
