@@ -47,20 +47,58 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region."""
+    """SM clock and throttle reasons DURING the timed region.  NVML is polled from a thread every ~0.5 ms (the timed
+    region of the small configs lasts a few ms, shorter than one `nvidia-smi -lms 100` poll); `nvidia-smi` is the
+    fallback when NVML cannot be loaded."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap"}
 
     def __init__(self, index: int):
         self.index, self.proc, self.lines = index, None, []
+        self.nvml, self.handle, self.thread, self.run = None, None, None, False
+        self.sm, self.mask, self.sm_max = [], 0, None
+
+    def _nvml_open(self):
+        import pynvml
+        pynvml.nvmlInit()
+        h = None
+        try:  # the CUDA ordinal is not the NVML index under CUDA_VISIBLE_DEVICES: go through the UUID
+            import torch
+            h = pynvml.nvmlDeviceGetHandleByUUID("GPU-" + str(torch.cuda.get_device_properties(self.index).uuid))
+        except Exception:
+            h = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+        self.sm_max = float(pynvml.nvmlDeviceGetMaxClockInfo(h, pynvml.NVML_CLOCK_SM))
+        pynvml.nvmlDeviceGetClockInfo(h, pynvml.NVML_CLOCK_SM)
+        self.nvml, self.handle = pynvml, h
+
+    def _poll(self):
+        nv, h = self.nvml, self.handle
+        while self.run:
+            try:
+                self.sm.append(float(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)))
+                self.mask |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+            except Exception:
+                pass
+            time.sleep(0.0005)
 
     def start(self):
+        """Called right before the timed region: only samples taken from here on count."""
+        try:
+            self._nvml_open()
+            self.run = True
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nvml = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
                                           "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
                                          stderr=subprocess.DEVNULL, text=True)
             threading.Thread(target=self._read, daemon=True).start()
+            time.sleep(0.3)
         except Exception:
             self.proc = None
 
@@ -69,6 +107,12 @@ class ClockSampler:
             self.lines.append(line.strip())
 
     def stop(self) -> dict:
+        if self.nvml is not None:
+            self.run = False
+            self.thread.join(timeout=1.0)
+            reasons = sorted(nm for bit, nm in self.REASONS.items() if self.mask & bit)
+            return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.sm_max,
+                    "reasons": reasons, "samples": len(self.sm), "source": "nvml"}
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         time.sleep(0.15)
@@ -87,7 +131,7 @@ class ClockSampler:
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "reasons": sorted(reasons), "samples": len(sm)}
+                "reasons": sorted(reasons), "samples": len(sm), "source": "nvidia-smi"}
 
 
 def make_workload(cfg: int, rank: int, scale: float):
@@ -202,22 +246,21 @@ def run_ours(args):
     inevt_frac = float((d_flags & 32).ne(0).float().mean().item())
 
     sampler = ClockSampler(local)
-    sampler.start()
-    time.sleep(0.3)
     B.prof_enable(True)
     l0 = B.launch_count()
     barrier()
+    sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(args.steps):
         step()
     e1.record()
     barrier()
+    clocks = sampler.stop()
     launches = B.launch_count() - l0
     ms_total = e0.elapsed_time(e1)
     stages = B.prof_read()
     B.prof_enable(False)
-    clocks = sampler.stop()
     ms_step = ms_total / args.steps
     from paper_1411_3968_b200 import sharding
 
@@ -249,6 +292,30 @@ def run_ours(args):
                 "launches_per_step": launches_dom, "kernel_ms_per_step": dur_ms,
                 "share_of_step": dur_ms / (ms_total / args.steps)}
     pipe_ach = ALG_BYTES_PIPELINE * n / (ms_total / args.steps * 1e-3) / 1e9  # this rank
+
+    # ---- level-0 N-in-TW trigger (tt_l0_ntw) on the sorted hits of this workload: timed on its
+    # own, NOT part of the step above.  N7TW1000 for the 32-PMT tower, N7TW500 otherwise.
+    # Algorithmic bytes: 16 B read (AoS record, only the time is used) + 1 B written per hit.
+    l0 = None
+    if rank == 0:
+        l0_n, l0_tw = 7, (1_000_000 if args.config == 0 else 500_000)
+        d_l0 = torch.empty(n, dtype=torch.uint8, device="cuda")
+        d_l0n = torch.zeros(1, dtype=torch.int32, device="cuda")
+        for _ in range(3):
+            B.tt_l0_ntw(d_out, seg, l0_n, l0_tw, d_l0, d_l0n)
+        torch.cuda.synchronize()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        for _ in range(args.steps):
+            B.tt_l0_ntw(d_out, seg, l0_n, l0_tw, d_l0, d_l0n)
+        a1.record()
+        torch.cuda.synchronize()
+        l0_ms = a0.elapsed_time(a1) / args.steps
+        l0_ach = 17.0 * n / (l0_ms * 1e-3) / 1e9
+        l0 = {"kernel": "l0_ntw_kernel", "multiplicity": l0_n, "window_ps": l0_tw, "ms": l0_ms,
+              "hits_per_s": n / (l0_ms * 1e-3), "alg_bytes_per_hit": 17, "achieved": l0_ach, "peak": peak,
+              "unit": "GB/s", "frac": l0_ach / peak, "n_start": int(d_l0n.cpu().numpy().view(np.uint32)[0])}
+        del d_l0
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
     e2e = None
@@ -312,6 +379,7 @@ def run_ours(args):
                                   "unit": "GB/s", "frac": pipe_ach / peak},
             "stages_ms_per_step": {k: round(v, 5) for k, v in sorted(per_stage.items())},
             "counters": counters,
+            "l0_ntw": l0,
             "e2e": e2e, "cpu_baseline": cpu,
         }
         print(json.dumps(out))

@@ -10,6 +10,7 @@
  *                      3 us), PAPER.md:61-64 (coincidences, QTRIG)       -- L1, L2, seed list
  *   tt_extract_events  PAPER.md:23 ("a 6 us time window ... centered at the time of the trigger seed"),
  *                      PAPER.md:67 ("all hits within +-3 us are tagged") -- event-window merge, tagging
+ *   tt_l0_ntw          PAPER.md:59, 67, 73 (N7TW1000 / N7TW500, the paper's level-0 trigger) -- N hits in TW
  *
  * Conventions
  *   d_*   device pointers (caller-owned; the library never allocates in the three hot calls)
@@ -79,6 +80,9 @@ enum {
 };
 #define TT_MAX_MULTIPLICITY 16
 #define TT_MAX_NEIGHBOURS 2048
+#define TT_MAX_L0_MULTIPLICITY 256
+/* per-hit byte of tt_l0_ntw */
+enum { TT_L0_START = 1, TT_L0_MEMBER = 2 };
 
 /* Causality table dtmax[pmt_a][pmt_b] in integer ps (BASELINE.json configs[0]: d_ij*n/c + 20 ns,
  * precomputed by the caller), block-sparse by tower pair:
@@ -124,6 +128,18 @@ int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_
                       tt_event* d_events, uint32_t event_cap, uint32_t* d_n_events, uint8_t* d_flags,
                       tt_hit* d_gather, uint32_t* d_n_gathered, void* d_ws, size_t* ws_bytes,
                       int32_t* d_status, void* stream);
+
+/* Level-0 N-in-TW trigger on time-sorted hits: "N7TW1000: looking for 7 hits
+ * in TW = 1000 ns: hit[i].time-hit[i+7].time< TW", PAPER.md:73 (N7TW500 for the 84-PMT tower), PAPER.md:67 (applied
+ * first, "as level 0 trigger").  Reading R14 / R20 of DESIGN.md: inside each segment, window start k fires <=> hit
+ * k + N - 1 exists in k's segment and t[k+N-1] - t[k] < window_ps (strict, as printed; window_ps <= 0 never fires).
+ * d_l0[n] (device, overwritten): TT_L0_START = the hit is a firing window start, TT_L0_MEMBER = the hit is one of the
+ * N hits k..k+N-1 of some firing window.  d_n_start (device, nullable): number of firing starts (zeroed by the call).
+ * d_sorted must be time-sorted inside each segment (the output of tt_sort_slice); unsorted input gives unspecified
+ * bits, never an out-of-bounds access.  multiplicity N in [1, TT_MAX_L0_MULTIPLICITY], else TT_E_INVAL.  No
+ * workspace, no status bits; asynchronous on `stream`. */
+int tt_l0_ntw(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
+              uint32_t multiplicity, int64_t window_ps, uint8_t* d_l0, uint32_t* d_n_start, void* stream);
 
 /* Whole-slice convenience with HOST buffers (end-to-end use and timing; not a hot call).
  * tt_host_ctx_create allocates, once, device buffers and workspaces for slices of up to max_n hits,
