@@ -132,3 +132,34 @@ def l0_ntw(sorted_hits: np.ndarray, seg_offsets: np.ndarray, *, multiplicity: in
     if rc != 0:
         raise ValueError("oracle_l0_ntw: invalid parameters")
     return l0, ns.value
+
+
+P_SC, P_FC, P_AFC, P_CAND_A, P_CAND_B = 1, 2, 4, 8, 16
+
+
+def pair_seeds(sorted_hits: np.ndarray, seg_offsets: np.ndarray, ppt: int, adj: np.ndarray, *, sc_window_ps=20_000,
+               fc_window_ps=100_000, afc_window_ps=250_000) -> np.ndarray:
+    """SC / FC / AFC bits per hit.  adj: (ppt, ppt) uint8, nonzero = adjacent PMTs of one tower."""
+    h = np.ascontiguousarray(sorted_hits, dtype=HIT)
+    seg = np.ascontiguousarray(seg_offsets, dtype=np.uint32)
+    a = np.ascontiguousarray(adj, dtype=np.uint8)
+    assert a.shape == (ppt, ppt)
+    bits = np.zeros(h.shape[0], dtype=np.uint8)
+    rc = lib().oracle_pair_seeds(_p(h), ctypes.c_uint32(h.shape[0]), _p(seg), ctypes.c_uint32(len(seg) - 1),
+                                 ctypes.c_uint32(int(ppt)), _p(a), ctypes.c_int64(int(sc_window_ps)),
+                                 ctypes.c_int64(int(fc_window_ps)), ctypes.c_int64(int(afc_window_ps)), _p(bits))
+    if rc != 0:
+        raise ValueError("oracle_pair_seeds: invalid parameters")
+    return bits
+
+
+def l0_combine(l0: np.ndarray, pair_bits: np.ndarray, multiplicity: int) -> np.ndarray:
+    """Candidate bits (8 = N-in-TW with [SC and AFC], 16 = with [FC and AFC]) on firing window starts."""
+    a = np.ascontiguousarray(l0, dtype=np.uint8)
+    b = np.ascontiguousarray(pair_bits, dtype=np.uint8)
+    assert a.shape == b.shape
+    out = np.zeros_like(a)
+    rc = lib().oracle_l0_combine(_p(a), _p(b), ctypes.c_uint32(a.shape[0]), ctypes.c_uint32(int(multiplicity)), _p(out))
+    if rc != 0:
+        raise ValueError("oracle_l0_combine: invalid input")
+    return out

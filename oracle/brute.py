@@ -124,3 +124,44 @@ def l0_ntw(h: np.ndarray, seg_offsets, N: int, tw_ps: int) -> np.ndarray:
                 out[i] |= 2
                 break
     return out
+
+
+def pair_seeds(h: np.ndarray, seg_offsets, ppt: int, adj: np.ndarray, w_sc: int, w_fc: int, w_afc: int) -> np.ndarray:
+    """PAPER.md:61-63 SC / FC / AFC straight from the sentences: all ordered pairs of a segment, no use of the time
+    order, one rule at a time."""
+    n = len(h)
+    sg = seg_id(n, seg_offsets)
+    t = [int(x) for x in h["t_ps"]]
+    pmt = [int(x) for x in h["pmt_id"]]
+    fl = [int(x) for x in h["floor"]]
+    out = np.zeros(n, dtype=np.uint8)
+    for i in range(n):
+        for j in range(n):
+            if i == j or sg[i] != sg[j] or pmt[i] == pmt[j]:
+                continue
+            dt = abs(t[i] - t[j])
+            tower_i, tower_j = pmt[i] // ppt, pmt[j] // ppt
+            # SC: "two hits occurred in two adjacent PMTs within 20 ns"
+            if dt <= w_sc and tower_i == tower_j and adj[pmt[i] % ppt][pmt[j] % ppt]:
+                out[i] |= 1
+            # FC: "two PMTs in the same floor within 100 ns"
+            if dt <= w_fc and fl[i] == fl[j]:
+                out[i] |= 2
+            # AFC: "two PMTs located at two consecutive floors within 250 ns"
+            if dt <= w_afc and tower_i == tower_j and abs(fl[i] - fl[j]) == 1:
+                out[i] |= 4
+    return out
+
+
+def l0_combine(l0: np.ndarray, pair_bits: np.ndarray, N: int) -> np.ndarray:
+    """PAPER.md:65 'applying N7TW1000, and if it is satisfied, we apply [SC and AFC] or [FC and AFC]'."""
+    out = np.zeros(len(l0), dtype=np.uint8)
+    for k in range(len(l0)):
+        if l0[k] & 1:
+            window = [int(b) for b in pair_bits[k:k + N]]
+            has = lambda bit: any(b & bit for b in window)
+            if has(1) and has(4):
+                out[k] |= 8
+            if has(2) and has(4):
+                out[k] |= 16
+    return out

@@ -17,6 +17,10 @@
 //                   pairwise L2 condition of north_star / BASELINE.json configs[0].
 //   oracle_events   PAPER.md:23 ("a 6 us time window ... centered at the time of the trigger
 //                   seed"), PAPER.md:67 ("all hits within +-3 us are tagged").
+//   oracle_pair_seeds  PAPER.md:61-63: SC ("two hits occurred in two adjacent PMTs within 20 ns"), FC ("two PMTs in the
+//                   same floor within 100 ns"), AFC ("two PMTs located at two consecutive floors within 250 ns").
+//   oracle_l0_combine  PAPER.md:65, 73: "applying N7TW1000, and if it is satisfied, we apply [SC and AFC] or [FC and
+//                   AFC]" (reading R22: evaluated over the N hits of each firing level-0 window).
 //   oracle_l0_ntw   PAPER.md:59 ("N7TW1000: looking for 7 hits in TW = 1000 ns:
 //                   hit[i].time-hit[i+7].time< TW"), PAPER.md:73 (N7TW500 for the 84-PMT tower)
 //                   (used first, "as level 0 trigger").  DESIGN.md reading R14: the printed formula has the
@@ -234,6 +238,65 @@ int oracle_l0_ntw(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n_
         }
     }
     *n_start = count;
+    return 0;
+}
+
+// Pair-coincidence seeds of the paper on time-sorted hits (readings R21, R4, R5).
+// For every ordered pair (i, j), j != i, of one segment with different pmt_id and |t_j - t_i| <= the rule's window
+// (inclusive, R4), hit i gets
+//   SC  (1): same tower (pmt_id / ppt) and adj[(pmt_i % ppt) * ppt + pmt_j % ppt] != 0   ("adjacent PMTs")
+//   FC  (2): same floor field                                                       ("same floor")
+//   AFC (4): same tower and floor fields that differ by exactly 1                   ("two consecutive floors")
+// The scan walks outwards from i in both directions while |dt| <= the largest window.
+int oracle_pair_seeds(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n_seg, uint32_t ppt,
+                      const uint8_t* adj, int64_t w_sc, int64_t w_fc, int64_t w_afc, uint8_t* bits) {
+    if (ppt < 1 || w_sc < 0 || w_fc < 0 || w_afc < 0) return -1;
+    for (uint32_t i = 0; i < n; ++i) bits[i] = 0;
+    const int64_t wmax = std::max(w_sc, std::max(w_fc, w_afc));
+    auto rules = [&](const Hit& a, const Hit& b, __int128 dt) -> uint8_t {
+        if (a.pmt_id == b.pmt_id) return 0;
+        uint8_t m = 0;
+        const bool same_tower = a.pmt_id / ppt == b.pmt_id / ppt;
+        if (dt <= w_sc && same_tower && adj[(size_t)(a.pmt_id % ppt) * ppt + b.pmt_id % ppt]) m |= 1;
+        if (dt <= w_fc && a.floor == b.floor) m |= 2;
+        const int df = (int)a.floor - (int)b.floor;
+        if (dt <= w_afc && same_tower && (df == 1 || df == -1)) m |= 4;
+        return m;
+    };
+    for (uint32_t s = 0; s < n_seg; ++s) {
+        const int64_t a = seg_off[s], b = seg_off[s + 1];
+        for (int64_t i = a; i < b; ++i) {
+            uint8_t m = 0;
+            for (int64_t j = i - 1; j >= a; --j) {
+                const __int128 dt = (__int128)h[i].t_ps - (__int128)h[j].t_ps;
+                if (dt > wmax) break;
+                m |= rules(h[i], h[j], dt);
+            }
+            for (int64_t j = i + 1; j < b; ++j) {
+                const __int128 dt = (__int128)h[j].t_ps - (__int128)h[i].t_ps;
+                if (dt > wmax) break;
+                m |= rules(h[i], h[j], dt);
+            }
+            bits[i] = m;
+        }
+    }
+    return 0;
+}
+
+// The paper's combined trigger (reading R22): for every firing level-0 window start k (l0[k] & 1; its
+// N hits k..k+N-1 lie in one segment), OR the pair bits of the N hits; out[k] gets 8 when both SC and AFC occur among
+// them ("N7TW with [SC and AFC]") and 16 when both FC and AFC occur ("N7TW with [FC and AFC]").  Other hits get 0.
+int oracle_l0_combine(const uint8_t* l0, const uint8_t* pair_bits, uint32_t n, uint32_t N, uint8_t* out) {
+    if (N < 1) return -1;
+    for (uint32_t k = 0; k < n; ++k) {
+        out[k] = 0;
+        if (!(l0[k] & 1)) continue;
+        if ((uint64_t)k + N > n) return -2;  // a start bit without its window: not an output of oracle_l0_ntw
+        uint8_t m = 0;
+        for (uint32_t j = k; j < k + N; ++j) m |= pair_bits[j];
+        if ((m & 1) && (m & 4)) out[k] |= 8;
+        if ((m & 2) && (m & 4)) out[k] |= 16;
+    }
     return 0;
 }
 

@@ -48,6 +48,21 @@ class Geometry:
     def n_pmt(self) -> int:
         return int(self.pos.shape[0])
 
+    def adjacency(self) -> np.ndarray:
+        """(ppt, ppt) uint8, 1 = "adjacent PMTs" (SC) of one tower -- DESIGN.md reading R21: two PMTs of
+        the same floor at that floor's smallest inter-PMT distance (cross arm: the two at 3*sqrt(2) m; bar: the
+        neighbours at 1.2 m).  Input data for tt_pair_seeds, like the causality table."""
+        ppt = self.pmts_per_tower
+        pos, fl = self.pos[:ppt], self.floor[:ppt]
+        d = np.linalg.norm(pos[:, None, :] - pos[None, :, :], axis=2)
+        same = (fl[:, None] == fl[None, :]) & ~np.eye(ppt, dtype=bool)
+        out = np.zeros((ppt, ppt), dtype=np.uint8)
+        for f in np.unique(fl):
+            m = same & (fl[:, None] == f)
+            if m.any():
+                out[m & (d <= d[m].min() + 1e-9)] = 1
+        return out
+
     def dense_table(self) -> np.ndarray:
         """(P,P) int32 table, -1 where the tower pair is unconnected (small geometries only)."""
         P, ppt = self.n_pmt, self.pmts_per_tower
