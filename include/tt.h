@@ -11,6 +11,8 @@
  *   tt_extract_events  PAPER.md:23 ("a 6 us time window ... centered at the time of the trigger seed"),
  *                      PAPER.md:67 ("all hits within +-3 us are tagged") -- event-window merge, tagging
  *   tt_l0_ntw          PAPER.md:59, 67, 73 (N7TW1000 / N7TW500, the paper's level-0 trigger) -- N hits in TW
+ *   tt_pair_seeds      PAPER.md:61-63 (SC, FC, AFC coincidences)          -- the paper's pair seeds
+ *   tt_l0_combine      PAPER.md:65, 73 (N7TW with [SC and AFC] or [FC and AFC]) -- the paper's combined trigger
  *
  * Conventions
  *   d_*   device pointers (caller-owned; the library never allocates in the three hot calls)
@@ -83,6 +85,8 @@ enum {
 #define TT_MAX_L0_MULTIPLICITY 256
 /* per-hit byte of tt_l0_ntw */
 enum { TT_L0_START = 1, TT_L0_MEMBER = 2 };
+/* per-hit byte of tt_pair_seeds (SC, FC, AFC) and of tt_l0_combine (CAND_A, CAND_B) */
+enum { TT_P_SC = 1, TT_P_FC = 2, TT_P_AFC = 4, TT_P_CAND_A = 8, TT_P_CAND_B = 16 };
 
 /* Causality table dtmax[pmt_a][pmt_b] in integer ps (BASELINE.json configs[0]: d_ij*n/c + 20 ns,
  * precomputed by the caller), block-sparse by tower pair:
@@ -140,6 +144,29 @@ int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_
  * workspace, no status bits; asynchronous on `stream`. */
 int tt_l0_ntw(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
               uint32_t multiplicity, int64_t window_ps, uint8_t* d_l0, uint32_t* d_n_start, void* stream);
+
+/* The paper's pair-coincidence seeds on time-sorted hits, PAPER.md:61-63:
+ *   TT_P_SC   "two hits occurred in two adjacent PMTs within 20 ns": same tower (pmt_id / pmts_per_tower) and
+ *             d_adj[(pmt_a % ppt) * ppt + pmt_b % ppt] != 0, |dt| <= sc_window_ps
+ *   TT_P_FC   "two PMTs in the same floor within 100 ns": equal `floor` fields, |dt| <= fc_window_ps
+ *   TT_P_AFC  "two PMTs located at two consecutive floors within 250 ns": same tower, `floor` fields differing by
+ *             exactly 1, |dt| <= afc_window_ps
+ * A pair is two hits of one segment on two DIFFERENT PMTs; windows are inclusive (readings R4, R5, R21).
+ * d_adj: device, uint8[ppt * ppt], symmetric, the caller's "adjacent PMTs" relation over one tower's PMTs.
+ * d_bits[n] (device, overwritten): OR of the rule bits over all partners of the hit.  Windows must be >= 0 and
+ * pmts_per_tower in [1, 65535], else TT_E_INVAL.  No workspace, no status bits; asynchronous on `stream`. */
+int tt_pair_seeds(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
+                  const uint8_t* d_adj, uint32_t pmts_per_tower, int64_t sc_window_ps, int64_t fc_window_ps,
+                  int64_t afc_window_ps, uint8_t* d_bits, void* stream);
+
+/* The paper's combined trigger, PAPER.md:65, 73 ("applying N7TW1000, and if it is satisfied, we apply [SC and AFC]
+ * or [FC and AFC] ... used to tag the muon track candidate"; reading R22): for every firing level-0 window
+ * start k (d_l0[k] & TT_L0_START, as written by tt_l0_ntw with the same multiplicity N), the pair bits of its N hits
+ * k..k+N-1 are OR-ed; d_cand[k] gets TT_P_CAND_A when SC and AFC both occur among them, TT_P_CAND_B when FC and AFC
+ * both occur.  Every other byte of d_cand[n] is 0.  d_n_cand (device, nullable, uint32[2], zeroed by the call):
+ * number of CAND_A and of CAND_B starts. */
+int tt_l0_combine(const uint8_t* d_l0, const uint8_t* d_pair_bits, uint32_t n, uint32_t multiplicity,
+                  uint8_t* d_cand, uint32_t* d_n_cand, void* stream);
 
 /* Whole-slice convenience with HOST buffers (end-to-end use and timing; not a hot call).
  * tt_host_ctx_create allocates, once, device buffers and workspaces for slices of up to max_n hits,

@@ -23,7 +23,7 @@ TT_S_SEED_OVERFLOW, TT_S_EVENT_OVERFLOW, TT_S_RUN_UNSORTED, TT_S_BAD_PMT, TT_S_D
 
 EXPORTS = ["tt_version", "tt_geometry_create", "tt_geometry_destroy", "tt_sort_slice", "tt_trigger_slice",
            "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host", "tt_launch_count",
-           "tt_prof_enable", "tt_prof_read", "tt_l0_ntw"]
+           "tt_prof_enable", "tt_prof_read", "tt_l0_ntw", "tt_pair_seeds", "tt_l0_combine"]
 
 HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
 EVENT_DTYPE = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
@@ -264,6 +264,49 @@ def l0_ntw(sorted_hits: np.ndarray, seg_offsets, multiplicity: int, window_ps: i
     tt_l0_ntw(d_sorted, seg, multiplicity, window_ps, d_l0, d_ns)
     torch.cuda.synchronize()
     return d_l0[:n].cpu().numpy(), int(d_ns.cpu().numpy().view(np.uint32)[0])
+
+
+TT_P_SC, TT_P_FC, TT_P_AFC, TT_P_CAND_A, TT_P_CAND_B = 1, 2, 4, 8, 16
+
+
+def tt_pair_seeds(d_sorted: torch.Tensor, seg: Offsets, d_adj: torch.Tensor, ppt: int, d_bits: torch.Tensor,
+                  sc_window_ps=20_000, fc_window_ps=100_000, afc_window_ps=250_000) -> None:
+    """Enqueue tt_pair_seeds (SC / FC / AFC): d_bits[n] uint8 receives TT_P_SC | TT_P_FC | TT_P_AFC."""
+    _need_cuda()
+    n = d_sorted.shape[0]
+    assert d_bits.dtype == torch.uint8 and d_bits.numel() >= n
+    assert d_adj.dtype == torch.uint8 and d_adj.numel() == ppt * ppt and d_adj.is_contiguous()
+    _check(load().tt_pair_seeds(_dp(d_sorted), c_u32(n), _dp(seg.d), c_u32(seg.count), _dp(d_adj), c_u32(int(ppt)),
+                                ctypes.c_int64(int(sc_window_ps)), ctypes.c_int64(int(fc_window_ps)),
+                                ctypes.c_int64(int(afc_window_ps)), _dp(d_bits), _stream()), "tt_pair_seeds")
+
+
+def tt_l0_combine(d_l0: torch.Tensor, d_pair_bits: torch.Tensor, n: int, multiplicity: int, d_cand: torch.Tensor,
+                  d_n_cand: torch.Tensor | None = None) -> None:
+    """Enqueue tt_l0_combine: d_cand[n] uint8 receives TT_P_CAND_A | TT_P_CAND_B on firing starts."""
+    _need_cuda()
+    assert d_cand.dtype == torch.uint8 and d_cand.numel() >= n
+    _check(load().tt_l0_combine(_dp(d_l0), _dp(d_pair_bits), c_u32(n), c_u32(int(multiplicity)), _dp(d_cand),
+                                _dp(d_n_cand), _stream()), "tt_l0_combine")
+
+
+def paper_trigger(sorted_hits: np.ndarray, seg_offsets, ppt: int, adj: np.ndarray, multiplicity: int, window_ps: int,
+                  sc_window_ps=20_000, fc_window_ps=100_000, afc_window_ps=250_000):
+    """Host-array convenience: tt_l0_ntw -> tt_pair_seeds -> tt_l0_combine.
+    Returns (l0 bytes, pair bits, candidate bytes, (n_start, n_cand_a, n_cand_b))."""
+    _need_cuda()
+    d_sorted = hits_to_device(sorted_hits)
+    seg = Offsets(seg_offsets)
+    n = d_sorted.shape[0]
+    d_adj = torch.from_numpy(np.ascontiguousarray(adj, dtype=np.uint8).reshape(-1).copy()).cuda()
+    d_l0, d_pb, d_cd = (torch.zeros(max(n, 1), dtype=torch.uint8, device="cuda") for _ in range(3))
+    d_cnt = torch.zeros(3, dtype=torch.int32, device="cuda")
+    tt_l0_ntw(d_sorted, seg, multiplicity, window_ps, d_l0, d_cnt[0:1])
+    tt_pair_seeds(d_sorted, seg, d_adj, ppt, d_pb, sc_window_ps, fc_window_ps, afc_window_ps)
+    tt_l0_combine(d_l0, d_pb, n, multiplicity, d_cd, d_cnt[1:3])
+    torch.cuda.synchronize()
+    cnt = d_cnt.cpu().numpy().view(np.uint32)
+    return d_l0[:n].cpu().numpy(), d_pb[:n].cpu().numpy(), d_cd[:n].cpu().numpy(), tuple(int(x) for x in cnt)
 
 
 @dataclass
