@@ -315,7 +315,36 @@ def run_ours(args):
         l0 = {"kernel": "l0_ntw_kernel", "multiplicity": l0_n, "window_ps": l0_tw, "ms": l0_ms,
               "hits_per_s": n / (l0_ms * 1e-3), "alg_bytes_per_hit": 17, "achieved": l0_ach, "peak": peak,
               "unit": "GB/s", "frac": l0_ach / peak, "n_start": int(d_l0n.cpu().numpy().view(np.uint32)[0])}
-        del d_l0
+        # the paper's pair seeds (SC / FC / AFC) and its combination with the level-0 windows
+        # (PAPER.md:65, 73): tt_pair_seeds 16 B read + 1 B written per hit, tt_l0_combine 2 B read + 1 B written
+        gw = w.geometry
+        d_adj = torch.from_numpy(gw.adjacency().reshape(-1).copy()).cuda()
+        d_pb = torch.empty(n, dtype=torch.uint8, device="cuda")
+        d_cd = torch.empty(n, dtype=torch.uint8, device="cuda")
+        d_nc = torch.zeros(2, dtype=torch.int32, device="cuda")
+
+        def timed(fn, reps):
+            fn()
+            torch.cuda.synchronize()
+            b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            b0.record()
+            for _ in range(reps):
+                fn()
+            b1.record()
+            torch.cuda.synchronize()
+            return b0.elapsed_time(b1) / reps
+
+        reps = max(2, min(args.steps, 5))
+        ps_ms = timed(lambda: B.tt_pair_seeds(d_out, seg, d_adj, gw.pmts_per_tower, d_pb), reps)
+        cb_ms = timed(lambda: B.tt_l0_combine(d_l0, d_pb, n, l0_n, d_cd, d_nc), reps)
+        nc = d_nc.cpu().numpy().view(np.uint32)
+        l0["pair_seeds"] = {"kernel": "pair_seeds_kernel", "windows_ps": [20_000, 100_000, 250_000], "ms": ps_ms,
+                            "alg_bytes_per_hit": 17, "achieved": 17.0 * n / (ps_ms * 1e-3) / 1e9, "peak": peak,
+                            "unit": "GB/s", "frac": 17.0 * n / (ps_ms * 1e-3) / 1e9 / peak}
+        l0["combine"] = {"kernel": "l0_combine_kernel", "ms": cb_ms, "alg_bytes_per_hit": 3,
+                         "achieved": 3.0 * n / (cb_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                         "frac": 3.0 * n / (cb_ms * 1e-3) / 1e9 / peak, "n_cand_a": int(nc[0]), "n_cand_b": int(nc[1])}
+        del d_l0, d_pb, d_cd
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
     e2e = None

@@ -25,6 +25,7 @@ constexpr uint32_t kPAdjSmem = 128;           // adjacency table in shared memor
 
 struct PairWin {
     uint64_t sc, fc, afc, wmax;
+    uint64_t rcp;  // ceil(2^32 / pmts_per_tower)
 };
 
 // rule bits of the ordered pair (i, j), dt = |t_j - t_i|; a = floor << 16 | local pmt, tw = tower
@@ -43,9 +44,11 @@ __device__ __forceinline__ uint32_t pair_rules(uint32_t ai, uint32_t twi, uint32
     return m;
 }
 
-__device__ __forceinline__ void split_pmt(uint32_t z, uint32_t ppt, uint32_t& a, uint32_t& tw) {
+// tower = pmt / ppt through the host's reciprocal rcp = ceil(2^32 / ppt): exact for pmt < 2^16 and ppt <= 2^16
+// (the error pmt * (rcp - 2^32 / ppt) < 2^16 <= 2^32 / ppt never reaches the next integer)
+__device__ __forceinline__ void split_pmt(uint32_t z, uint32_t ppt, uint64_t rcp, uint32_t& a, uint32_t& tw) {
     const uint32_t pmt = z & 0xFFFFu;
-    tw = pmt / ppt;
+    tw = (uint32_t)(((uint64_t)pmt * rcp) >> 32);
     a = (z & 0xFFFF0000u) | (pmt - tw * ppt);
 }
 
@@ -61,7 +64,7 @@ __device__ uint32_t pair_scan_global(const uint4* __restrict__ hits, int64_t t, 
         const uint64_t dt = udiff(t, hit_time(v));
         if (dt > w.wmax) break;
         uint32_t aj, twj;
-        split_pmt(v.z, ppt, aj, twj);
+        split_pmt(v.z, ppt, w.rcp, aj, twj);
         m |= pair_rules<uint64_t>(ai, twi, aj, twj, dt, w.sc, w.fc, w.afc, ppt, ga);
     }
     for (uint32_t j = above; j < b; ++j) {
@@ -69,7 +72,7 @@ __device__ uint32_t pair_scan_global(const uint4* __restrict__ hits, int64_t t, 
         const uint64_t dt = udiff(hit_time(v), t);
         if (dt > w.wmax) break;
         uint32_t aj, twj;
-        split_pmt(v.z, ppt, aj, twj);
+        split_pmt(v.z, ppt, w.rcp, aj, twj);
         m |= pair_rules<uint64_t>(ai, twi, aj, twj, dt, w.sc, w.fc, w.afc, ppt, ga);
     }
     return m;
@@ -116,7 +119,7 @@ __global__ void __launch_bounds__(kPThreads) pair_seeds_kernel(const uint4* __re
             const uint64_t d64 = udiff(hit_time(v), t0);
             wide |= d64 >= 0xFFFFFFFFull;
             tr = (uint32_t)d64;
-            split_pmt(v.z, ppt, a, tw);
+            split_pmt(v.z, ppt, w.rcp, a, tw);
         }
         sm.t[e] = tr; sm.a[e] = a; sm.tw[e] = tw;
     }
@@ -179,7 +182,7 @@ __global__ void __launch_bounds__(kPThreads) pair_seeds_kernel(const uint4* __re
             }
             const uint4 v = __ldg(hits + g);
             uint32_t ai, twi;
-            split_pmt(v.z, ppt, ai, twi);
+            split_pmt(v.z, ppt, w.rcp, ai, twi);
             const uint32_t mine = pair_scan_global(hits, hit_time(v), ai, twi, g, g + 1, sa, sb, w, ppt, adj);
             if (mine) atomicOr(&sm.f[(e - kPHalo) >> 2], mine << (8 * ((e - kPHalo) & 3)));
         }
@@ -197,29 +200,70 @@ __global__ void __launch_bounds__(kPThreads) pair_seeds_kernel(const uint4* __re
 }
 
 // The combined trigger on firing level-0 window starts (reading R22): OR of the pair bits of the N hits k..k+N-1.
-// One thread per hit; the window bytes are neighbouring threads' own bytes, so the reads hit L1.
+// One CTA per tile of kCTile hits: the tile's pair bytes and the N - 1 bytes behind it are staged in shared memory,
+// lanes take consecutive hits (their window bytes are consecutive: conflict-free reads), the result bytes go back
+// through shared memory so that every thread writes 16 of them at once; one pair of atomics per CTA for the counts.
 constexpr int kCThreads = 256;
+constexpr int kCPer = 16;
+constexpr int kCTile = kCThreads * kCPer;  // 4096
 __global__ void __launch_bounds__(kCThreads) l0_combine_kernel(const uint8_t* __restrict__ l0,
                                                                const uint8_t* __restrict__ pair_bits, uint32_t n,
                                                                uint32_t N, uint8_t* __restrict__ cand,
                                                                uint32_t* __restrict__ n_cand) {
-    const uint32_t k = blockIdx.x * (uint32_t)kCThreads + threadIdx.x;
-    uint32_t out = 0;
-    if (k < n && (l0[k] & TT_L0_START)) {
-        uint32_t m = 0;
-        const uint32_t end = (uint64_t)k + N < (uint64_t)n ? k + N : n;  // a start from tt_l0_ntw has its whole window
-        for (uint32_t j = k; j < end; ++j) m |= pair_bits[j];
-        if ((m & TT_P_SC) && (m & TT_P_AFC)) out |= TT_P_CAND_A;
-        if ((m & TT_P_FC) && (m & TT_P_AFC)) out |= TT_P_CAND_B;
-    }
-    if (k < n) cand[k] = (uint8_t)out;
-    if (n_cand) {
-        const uint32_t ca = __popc(__ballot_sync(0xffffffffu, out & TT_P_CAND_A));
-        const uint32_t cb = __popc(__ballot_sync(0xffffffffu, out & TT_P_CAND_B));
-        if ((threadIdx.x & 31) == 0) {
-            if (ca) atomicAdd(n_cand, ca);
-            if (cb) atomicAdd(n_cand + 1, cb);
+    __shared__ __align__(16) uint8_t s_pb[kCTile + TT_MAX_L0_MULTIPLICITY];
+    __shared__ __align__(16) uint8_t s_l0[kCTile];
+    __shared__ __align__(16) uint8_t s_out[kCTile];
+    __shared__ uint32_t s_cnt[2];
+    const uint32_t tid = threadIdx.x;
+    const uint32_t tb = blockIdx.x * (uint32_t)kCTile;
+    const uint32_t te = min(n, tb + (uint32_t)kCTile);
+    const uint32_t i0 = tb + tid * kCPer;
+    if (tid < 2) s_cnt[tid] = 0;
+    // stage: 16 bytes per thread of both arrays (vector loads when the pointers allow), then the halo of pair bytes
+    const bool full = i0 + kCPer <= te;
+    if (full && ((((uintptr_t)(pair_bits + i0)) | ((uintptr_t)(l0 + i0))) & 15) == 0) {
+        reinterpret_cast<uint4*>(s_pb)[tid] = __ldg(reinterpret_cast<const uint4*>(pair_bits + i0));
+        reinterpret_cast<uint4*>(s_l0)[tid] = __ldg(reinterpret_cast<const uint4*>(l0 + i0));
+    } else {
+        for (uint32_t b8 = 0; b8 < (uint32_t)kCPer; ++b8) {
+            const uint32_t i = i0 + b8;
+            s_pb[tid * kCPer + b8] = i < te ? pair_bits[i] : (uint8_t)0;
+            s_l0[tid * kCPer + b8] = i < te ? l0[i] : (uint8_t)0;
         }
+    }
+    for (uint32_t h = tid; h + 1 < N; h += kCThreads) {  // N - 1 bytes behind the tile
+        const uint32_t i = tb + (uint32_t)kCTile + h;
+        s_pb[kCTile + h] = i < n ? pair_bits[i] : (uint8_t)0;
+    }
+    __syncthreads();
+    uint32_t ca = 0, cb = 0;
+#pragma unroll 4
+    for (int r = 0; r < kCPer; ++r) {
+        const uint32_t q = tid + r * kCThreads;  // lanes on consecutive hits
+        uint32_t out = 0;
+        if (tb + q < te && (s_l0[q] & TT_L0_START)) {
+            uint32_t m = 0;
+            for (uint32_t j = 0; j < N; ++j) m |= s_pb[q + j];  // bytes past n are 0: a start from tt_l0_ntw never needs them
+            if ((m & TT_P_SC) && (m & TT_P_AFC)) { out |= TT_P_CAND_A; ++ca; }
+            if ((m & TT_P_FC) && (m & TT_P_AFC)) { out |= TT_P_CAND_B; ++cb; }
+        }
+        s_out[q] = (uint8_t)out;
+    }
+    __syncthreads();
+    if (full && (((uintptr_t)(cand + i0)) & 15) == 0) {
+        *reinterpret_cast<uint4*>(cand + i0) = reinterpret_cast<const uint4*>(s_out)[tid];
+    } else {
+        for (uint32_t b8 = 0; b8 < (uint32_t)kCPer && i0 + b8 < te; ++b8) cand[i0 + b8] = s_out[tid * kCPer + b8];
+    }
+    if (n_cand) {
+        ca = __reduce_add_sync(0xffffffffu, ca);
+        cb = __reduce_add_sync(0xffffffffu, cb);
+        if ((tid & 31) == 0) {
+            if (ca) atomicAdd(&s_cnt[0], ca);
+            if (cb) atomicAdd(&s_cnt[1], cb);
+        }
+        __syncthreads();
+        if (tid < 2 && s_cnt[tid]) atomicAdd(n_cand + tid, s_cnt[tid]);
     }
 }
 
@@ -239,6 +283,7 @@ extern "C" int tt_pair_seeds(const tt_hit* d_sorted, uint32_t n, const uint32_t*
     w.sc = (uint64_t)sc_window_ps; w.fc = (uint64_t)fc_window_ps; w.afc = (uint64_t)afc_window_ps;
     w.wmax = w.sc > w.fc ? w.sc : w.fc;
     w.wmax = w.afc > w.wmax ? w.afc : w.wmax;
+    w.rcp = ((1ull << 32) + pmts_per_tower - 1) / pmts_per_tower;
     const size_t smem = sizeof(PairSmem) + (pmts_per_tower <= kPAdjSmem ? (size_t)pmts_per_tower * pmts_per_tower : 0);
     static bool attr_done = false;
     if (!attr_done) {
@@ -263,7 +308,7 @@ extern "C" int tt_l0_combine(const uint8_t* d_l0, const uint8_t* d_pair_bits, ui
     if (d_n_cand) TT_CUDA_OK(cudaMemsetAsync(d_n_cand, 0, 2 * sizeof(uint32_t), s));
     if (n == 0) return TT_OK;
     prof_mark(s, "pairs.combine");
-    TT_K(l0_combine_kernel)<<<div_up(n, kCThreads), kCThreads, 0, s>>>(d_l0, d_pair_bits, n, multiplicity, d_cand, d_n_cand);
+    TT_K(l0_combine_kernel)<<<div_up(n, kCTile), kCThreads, 0, s>>>(d_l0, d_pair_bits, n, multiplicity, d_cand, d_n_cand);
     prof_end(s);
     TT_LAUNCH_OK();
     return TT_OK;
