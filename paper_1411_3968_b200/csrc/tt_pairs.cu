@@ -21,6 +21,7 @@ constexpr int kPPer = 8;
 constexpr int kPTile = kPThreads * kPPer;     // 2048
 constexpr int kPHalo = 256;
 constexpr int kPStage = kPTile + 2 * kPHalo;  // 2560
+constexpr int kPPad = 64;                     // readable slack behind the staged arrays (speculative lockstep reads)
 constexpr uint32_t kPAdjSmem = 128;           // adjacency table in shared memory up to 128 PMTs per tower (16 KB)
 
 struct PairWin {
@@ -79,9 +80,9 @@ __device__ uint32_t pair_scan_global(const uint4* __restrict__ hits, int64_t t, 
 }
 
 struct PairSmem {
-    uint32_t t[kPStage];    // time relative to the first staged hit
-    uint32_t a[kPStage];    // floor << 16 | local pmt
-    uint32_t tw[kPStage];   // tower
+    uint32_t t[kPStage + kPPad];    // time relative to the first staged hit
+    uint32_t a[kPStage + kPPad];    // floor << 16 | local pmt
+    uint32_t tw[kPStage + kPPad];   // tower
     uint32_t f[kPTile / 4]; // rule bytes of the in-tile hits
 };
 
@@ -96,9 +97,18 @@ __global__ void __launch_bounds__(kPThreads) pair_seeds_kernel(const uint4* __re
     const uint32_t tid = threadIdx.x;
     const uint32_t tb = blockIdx.x * (uint32_t)kPTile;
     const uint32_t te = min(n, tb + (uint32_t)kPTile);
-    const uint32_t glo = tb >= (uint32_t)kPHalo ? tb - kPHalo : 0u;
-    const uint32_t ghi = min(n, te + (uint32_t)kPHalo);
-    const uint32_t g0 = tb - (uint32_t)kPHalo;  // staged slot e <-> global index g0 + e (modulo 2^32)
+    // Staged halo: 32 hits when the 32nd hit before and after the tile already lies outside the largest window (the
+    // usual case: a tower has a hit or two inside 250 ns), else kPHalo.  Purely a cost choice: whatever the staged
+    // range cannot decide goes to the exact global scans below, so the result does not depend on it.
+    uint32_t halo = kPHalo;
+    if (tb >= 32u && te + 32u <= n) {
+        const int64_t f0 = hit_time(__ldg(hits + (tb - 32u))), f1 = hit_time(__ldg(hits + tb));
+        const int64_t b0 = hit_time(__ldg(hits + (te - 1u))), b1 = hit_time(__ldg(hits + (te + 31u)));
+        if (f1 >= f0 && b1 >= b0 && udiff(f1, f0) > w.wmax && udiff(b1, b0) > w.wmax) halo = 32u;
+    }
+    const uint32_t glo = tb >= halo ? tb - halo : 0u;
+    const uint32_t ghi = min(n, te + halo);
+    const uint32_t g0 = tb - (uint32_t)kPHalo;  // staged slot e <-> global index g0 + e (modulo 2^32), whatever the halo
     const uint32_t e_lo = glo - g0, e_hi = ghi - g0, e_te = te - g0;
     uint32_t seg_a = 0, seg_b = n;
     bool one_seg = true;
@@ -124,6 +134,7 @@ __global__ void __launch_bounds__(kPThreads) pair_seeds_kernel(const uint4* __re
         sm.t[e] = tr; sm.a[e] = a; sm.tw[e] = tw;
     }
     for (uint32_t i = tid; i < (uint32_t)kPTile / 4; i += kPThreads) sm.f[i] = 0;
+    if (tid < (uint32_t)kPPad) { sm.t[kPStage + tid] = 0xFFFFFFFFu; sm.a[kPStage + tid] = 0xFFFFFFFFu; sm.tw[kPStage + tid] = 0xFFFFFFFFu; }
     if (adj_smem)
         for (uint32_t i = tid; i < ppt * ppt; i += kPThreads) s_adj[i] = __ldg(adj + i);
     const bool fits32 = !__syncthreads_or(wide);
@@ -131,31 +142,55 @@ __global__ void __launch_bounds__(kPThreads) pair_seeds_kernel(const uint4* __re
     const uint32_t w_sc = clamp32(w.sc), w_fc = clamp32(w.fc), w_afc = clamp32(w.afc), w_max = clamp32(w.wmax);
     auto sa_ = [&](uint32_t k) { return adj_smem ? s_adj[k] != 0 : __ldg(adj + k) != 0; };
     if (fits32) {
-        // rounds 0: the halo before the tile (marks its in-tile partners only); rounds 1..: the tile
+        // round 0: the halo before the tile (marks its in-tile partners only); rounds 1..: the tile.  A warp walks its 32
+        // hits in lockstep, four offsets per step, and leaves when no lane has an offset inside its window any more.
+        // Prefilter per offset: a rule needs floors within one of each other (FC, AFC) or dt inside the SC window.
+        const uint32_t lane = tid & 31u;
 #pragma unroll 1
         for (int r = 0; r < (kPTile + kPHalo) / kPThreads; ++r) {
             const uint32_t e = tid + r * kPThreads;
-            if (e < e_lo || e >= e_te) continue;
+            const uint32_t w0 = e - lane;
+            if (w0 >= e_te) break;                 // warp-uniform
+            if (w0 + 32u <= e_lo) continue;        // warp-uniform: nothing staged here
+            const bool valid = e >= e_lo && e < e_te;
             const uint32_t ti = sm.t[e], ai = sm.a[e], twi = sm.tw[e];
             uint32_t jmax = e_hi, sa = seg_a, sb = seg_b;
-            if (!one_seg) {
+            if (!one_seg && valid) {
                 const uint32_t s = find_segment(seg_off, n_seg, g0 + e);
                 sa = __ldg(seg_off + s);
                 sb = __ldg(seg_off + s + 1);
                 if (sb < ghi) jmax = sb - g0;
             }
             uint32_t mine = 0;
-            uint32_t j = e + 1;
-            for (; j < jmax; ++j) {
-                const uint32_t dt = sm.t[j] - ti;
-                if (dt > w_max) break;
-                const uint32_t m = pair_rules<uint32_t>(ai, twi, sm.a[j], sm.tw[j], dt, w_sc, w_fc, w_afc, ppt, sa_);
-                if (m) {
-                    mine |= m;
-                    if (j >= (uint32_t)kPHalo && j < e_te)
-                        atomicOr(&sm.f[(j - kPHalo) >> 2], m << (8 * ((j - kPHalo) & 3)));
+            const uint32_t fi1 = (ai >> 16) - 1u;  // floor - 1: (floor_j - fi1) <= 2 <=> floors within one of each other
+            for (uint32_t d0 = 1;; d0 += 4) {
+                const uint32_t j0 = e + d0;
+                const uint32_t dt0 = sm.t[j0] - ti;
+                if (!__any_sync(0xffffffffu, valid && j0 < jmax && dt0 <= w_max)) break;
+                const uint32_t dt1 = sm.t[j0 + 1] - ti, dt2 = sm.t[j0 + 2] - ti, dt3 = sm.t[j0 + 3] - ti;
+                const uint32_t a0 = sm.a[j0], a1 = sm.a[j0 + 1], a2 = sm.a[j0 + 2], a3 = sm.a[j0 + 3];
+                const bool p0 = valid && j0 < jmax && dt0 <= w_max && ((a0 >> 16) - fi1 <= 2u || dt0 <= w_sc);
+                const bool p1 = valid && j0 + 1 < jmax && dt1 <= w_max && ((a1 >> 16) - fi1 <= 2u || dt1 <= w_sc);
+                const bool p2 = valid && j0 + 2 < jmax && dt2 <= w_max && ((a2 >> 16) - fi1 <= 2u || dt2 <= w_sc);
+                const bool p3 = valid && j0 + 3 < jmax && dt3 <= w_max && ((a3 >> 16) - fi1 <= 2u || dt3 <= w_sc);
+                if (p0 | p1 | p2 | p3) {
+                    const uint32_t pm = (p0 ? 1u : 0u) | (p1 ? 2u : 0u) | (p2 ? 4u : 0u) | (p3 ? 8u : 0u);
+#pragma unroll
+                    for (uint32_t q = 0; q < 4; ++q) {
+                        if (!((pm >> q) & 1u)) continue;
+                        const uint32_t j = j0 + q;
+                        const uint32_t m = pair_rules<uint32_t>(ai, twi, sm.a[j], sm.tw[j], sm.t[j] - ti, w_sc, w_fc, w_afc, ppt, sa_);
+                        if (m) {
+                            mine |= m;
+                            if (j >= (uint32_t)kPHalo && j < e_te)
+                                atomicOr(&sm.f[(j - kPHalo) >> 2], m << (8 * ((j - kPHalo) & 3)));
+                        }
+                    }
                 }
             }
+            if (!valid) continue;
+            // the staged hits of this hit's segment end inside its window <=> the last of them is still inside
+            const uint32_t j = (jmax - 1u > e && sm.t[jmax - 1u] - ti > w_max) ? 0u : jmax;  // == jmax: not closed
             if (e < (uint32_t)kPHalo) continue;  // a halo hit: its own bits belong to another tile
             // what the staged window leaves open: partners beyond its end / before its start
             const bool open_fwd = j == jmax && jmax == e_hi && ghi < sb;
