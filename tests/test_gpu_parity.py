@@ -317,3 +317,43 @@ def test_many_towers_global_pair_table(B, oracle_lib):
     r = B.process_slice(h, seg, runs, _geo(B, geo), _prm(B, p))
     _compare(r, o)
     assert r.status == 0 and len(o["seeds"]) > 0
+
+
+@pytest.mark.parametrize("cfg,ts,ss", [(2, 0.01, 1), (3, 0.02, 8 / 64), (4, 0.004, 1)])
+def test_reused_dirty_workspaces_and_determinism(cfg, ts, ss, B, oracle_lib):
+    """bench.py reuses its workspaces and output buffers from step to step: garbage-filled workspaces and outputs,
+    three consecutive runs of the three calls, every run byte-identical to the oracle (hence to each other)."""
+    w = W.make_config(cfg, time_scale=ts, seg_scale=ss)
+    p = w.params
+    o = oracle_chain(w.hits, w.seg_offsets, w.geometry, p)
+    n = w.n
+    geo, prm = _geo(B, w.geometry), _prm(B, p)
+    seg, runs = B.Offsets(w.seg_offsets), B.Offsets(w.run_offsets)
+    d_in = B.hits_to_device(w.hits)
+    d_out = torch.full_like(d_in, -1)
+    d_perm = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    d_flags = torch.full((n,), 0xFF, dtype=torch.uint8, device="cuda")
+    d_seeds = torch.full((n,), -1, dtype=torch.int32, device="cuda")
+    d_ev = torch.full((n, 4), -1, dtype=torch.int64, device="cuda")
+    d_cnt = torch.full((4,), -1, dtype=torch.int32, device="cuda")
+    ws = {}
+    for it in range(3):
+        d_cnt[2] = 0  # the status word is the caller's to clear
+        for k in ("s", "t", "e"):
+            if k in ws:
+                ws[k].fill_(0xA5 if it == 1 else 0xFF)  # dirty workspaces: nothing may rely on their content
+        ws["s"] = B.tt_sort_slice(d_in, d_out, d_perm, seg, runs, d_cnt[2:3], ws.get("s"))
+        ws["t"] = B.tt_trigger_slice(d_out, seg, geo, prm, d_flags, d_seeds, d_cnt[0:1], d_cnt[2:3], ws.get("t"))
+        ws["e"] = B.tt_extract_events(d_out, seg, d_seeds, d_cnt[0:1], prm, d_ev, d_cnt[1:2], d_flags, None, None,
+                                      d_cnt[2:3], ws.get("e"))
+        torch.cuda.synchronize()
+        cnt = d_cnt.cpu().numpy().view(np.uint32)
+        ns, ne, status = int(cnt[0]), int(cnt[1]), int(cnt[2])
+        assert status == 0, (it, status)
+        assert B.hits_to_host(d_out).tobytes() == o["sorted"].tobytes(), it
+        assert (d_perm.cpu().numpy().view(np.uint32) == o["perm"]).all(), it
+        assert (d_flags.cpu().numpy() == o["flags"]).all(), it
+        assert ns == len(o["seeds"]) and (d_seeds[:ns].cpu().numpy().view(np.uint32) == o["seeds"]).all(), it
+        ev = d_ev[:ne].cpu().numpy().reshape(-1).view(B.EVENT_DTYPE)
+        assert ne == len(o["events"]) and ev.tobytes() == o["events"].tobytes(), it
+    geo.close()
