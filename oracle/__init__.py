@@ -163,3 +163,18 @@ def l0_combine(l0: np.ndarray, pair_bits: np.ndarray, multiplicity: int) -> np.n
     if rc != 0:
         raise ValueError("oracle_l0_combine: invalid input")
     return out
+
+
+def l0_dntw(sorted_hits: np.ndarray, seg_offsets: np.ndarray, *, multiplicity: int, window_ps: int):
+    """Distinct-PMT level-0 trigger DNnTW -> (l0 bytes [n], number of firing window starts)."""
+    h = np.ascontiguousarray(sorted_hits, dtype=HIT)
+    seg = np.ascontiguousarray(seg_offsets, dtype=np.uint32)
+    n = h.shape[0]
+    l0 = np.zeros(n, dtype=np.uint8)
+    ns = ctypes.c_uint32(0)
+    rc = lib().oracle_l0_dntw(_p(h), ctypes.c_uint32(n), _p(seg), ctypes.c_uint32(len(seg) - 1),
+                              ctypes.c_uint32(int(multiplicity)), ctypes.c_int64(int(window_ps)), _p(l0),
+                              ctypes.byref(ns))
+    if rc != 0:
+        raise ValueError("oracle_l0_dntw: invalid parameters")
+    return l0, ns.value

@@ -165,3 +165,23 @@ def l0_combine(l0: np.ndarray, pair_bits: np.ndarray, N: int) -> np.ndarray:
             if has(2) and has(4):
                 out[k] |= 16
     return out
+
+
+def l0_dntw(h: np.ndarray, seg_offsets, N: int, tw_ps: int) -> np.ndarray:
+    """PAPER.md:60 'N hits from different PMTs within TW'.  Set formulation: start k fires <=> the set of pmt_id over
+    the hits of its segment with index >= k and t < t_k + TW has at least N elements; its members run from k to the
+    smallest index e for which the set over [k, e] already has N elements."""
+    n = len(h)
+    sg = seg_id(n, seg_offsets)
+    t = [int(x) for x in h["t_ps"]]
+    pmt = [int(x) for x in h["pmt_id"]]
+    out = np.zeros(n, dtype=np.uint8)
+    for k in range(n):
+        inside = [j for j in range(k, n) if sg[j] == sg[k] and t[j] < t[k] + tw_ps]
+        if tw_ps <= 0 or len({pmt[j] for j in inside}) < N:
+            continue
+        e = next(j for j in inside if len({pmt[m] for m in inside if m <= j}) >= N)
+        out[k] |= 1
+        for m in range(k, e + 1):
+            out[m] |= 2
+    return out

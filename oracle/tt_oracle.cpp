@@ -21,6 +21,8 @@
 //                   same floor within 100 ns"), AFC ("two PMTs located at two consecutive floors within 250 ns").
 //   oracle_l0_combine  PAPER.md:65, 73: "applying N7TW1000, and if it is satisfied, we apply [SC and AFC] or [FC and
 //                   AFC]" (reading R22: evaluated over the N hits of each firing level-0 window).
+//   oracle_l0_dntw  PAPER.md:60 ("DN7TW1000: looking for 7 hits from different PMTs within TW = 1000 ns"); DESIGN.md
+//                   reading R23.
 //   oracle_l0_ntw   PAPER.md:59 ("N7TW1000: looking for 7 hits in TW = 1000 ns:
 //                   hit[i].time-hit[i+7].time< TW"), PAPER.md:73 (N7TW500 for the 84-PMT tower)
 //                   (used first, "as level 0 trigger").  DESIGN.md reading R14: the printed formula has the
@@ -297,6 +299,37 @@ int oracle_l0_combine(const uint8_t* l0, const uint8_t* pair_bits, uint32_t n, u
         if ((m & 1) && (m & 4)) out[k] |= 8;
         if ((m & 2) && (m & 4)) out[k] |= 16;
     }
+    return 0;
+}
+
+// Distinct-PMT level-0 trigger (reading R23).  Inside each segment, window start k fires <=> the hits
+// j >= k with t_j - t_k < TW (strict, as for N-in-TW) carry at least N different pmt_id values.  Its members are the
+// hits k..e_k, e_k = the first hit at which the N-th different PMT appears (with all PMTs different this is the plain
+// N-in-TW window k..k+N-1).  l0[i]: 1 = firing start, 2 = member of some firing window; *n_start = firing starts.
+int oracle_l0_dntw(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n_seg, uint32_t N, int64_t TW,
+                   uint8_t* l0, uint32_t* n_start) {
+    if (N < 1) return -1;
+    for (uint32_t i = 0; i < n; ++i) l0[i] = 0;
+    uint32_t count = 0;
+    std::vector<uint16_t> seen;
+    for (uint32_t s = 0; s < n_seg; ++s) {
+        const uint64_t a = seg_off[s], b = seg_off[s + 1];
+        for (uint64_t k = a; k < b; ++k) {
+            seen.clear();
+            for (uint64_t j = k; j < b; ++j) {
+                const __int128 dt = (__int128)h[j].t_ps - (__int128)h[k].t_ps;
+                if (!(dt < (__int128)TW)) break;
+                if (std::find(seen.begin(), seen.end(), h[j].pmt_id) == seen.end()) seen.push_back(h[j].pmt_id);
+                if (seen.size() == N) {
+                    l0[k] |= 1;
+                    for (uint64_t m = k; m <= j; ++m) l0[m] |= 2;
+                    ++count;
+                    break;
+                }
+            }
+        }
+    }
+    *n_start = count;
     return 0;
 }
 
