@@ -11,6 +11,7 @@
  *   tt_extract_events  PAPER.md:23 ("a 6 us time window ... centered at the time of the trigger seed"),
  *                      PAPER.md:67 ("all hits within +-3 us are tagged") -- event-window merge, tagging
  *   tt_l0_ntw          PAPER.md:59, 67, 73 (N7TW1000 / N7TW500, the paper's level-0 trigger) -- N hits in TW
+ *   tt_l0_dntw         PAPER.md:60 (DN7TW1000: N hits from different PMTs in TW)   -- distinct-PMT level-0 trigger
  *   tt_pair_seeds      PAPER.md:61-63 (SC, FC, AFC coincidences)          -- the paper's pair seeds
  *   tt_l0_combine      PAPER.md:65, 73 (N7TW with [SC and AFC] or [FC and AFC]) -- the paper's combined trigger
  *
@@ -83,6 +84,7 @@ enum {
 #define TT_MAX_MULTIPLICITY 16
 #define TT_MAX_NEIGHBOURS 2048
 #define TT_MAX_L0_MULTIPLICITY 256
+#define TT_MAX_DN_MULTIPLICITY 16
 /* per-hit byte of tt_l0_ntw */
 enum { TT_L0_START = 1, TT_L0_MEMBER = 2 };
 /* per-hit byte of tt_pair_seeds (SC, FC, AFC) and of tt_l0_combine (CAND_A, CAND_B) */
@@ -144,6 +146,17 @@ int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_
  * workspace, no status bits; asynchronous on `stream`. */
 int tt_l0_ntw(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
               uint32_t multiplicity, int64_t window_ps, uint8_t* d_l0, uint32_t* d_n_start, void* stream);
+
+/* Distinct-PMT level-0 trigger DNnTW (rest of SURVEY.md 8(f) NEXT-1): "DN7TW1000: looking for 7 hits
+ * from different PMTs within TW = 1000 ns".  Reading R23 of DESIGN.md: inside each segment, window start k fires <=> the
+ * hits j >= k with t_j - t_k < window_ps (strict) carry at least N different pmt_id values; its members are the hits
+ * k..e_k, e_k = the first hit at which the N-th different PMT appears (with all PMTs different: tt_l0_ntw's window).
+ * d_l0[n] (device; zeroed, then written, by the call): TT_L0_START | TT_L0_MEMBER as for tt_l0_ntw.  d_n_start
+ * (device, nullable): number of firing starts.  multiplicity N in [1, TT_MAX_DN_MULTIPLICITY], else TT_E_INVAL.
+ * Exact for any hit density (windows longer than the staged tile are finished from global memory).  No workspace, no
+ * status bits; asynchronous on `stream`. */
+int tt_l0_dntw(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
+               uint32_t multiplicity, int64_t window_ps, uint8_t* d_l0, uint32_t* d_n_start, void* stream);
 
 /* The paper's pair-coincidence seeds on time-sorted hits, PAPER.md:61-63:
  *   TT_P_SC   "two hits occurred in two adjacent PMTs within 20 ns": same tower (pmt_id / pmts_per_tower) and

@@ -23,7 +23,8 @@ TT_S_SEED_OVERFLOW, TT_S_EVENT_OVERFLOW, TT_S_RUN_UNSORTED, TT_S_BAD_PMT, TT_S_D
 
 EXPORTS = ["tt_version", "tt_geometry_create", "tt_geometry_destroy", "tt_sort_slice", "tt_trigger_slice",
            "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host", "tt_launch_count",
-           "tt_prof_enable", "tt_prof_read", "tt_l0_ntw", "tt_pair_seeds", "tt_l0_combine"]
+           "tt_prof_enable", "tt_prof_read", "tt_l0_ntw", "tt_pair_seeds", "tt_l0_combine",
+           "tt_l0_dntw"]
 
 HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
 EVENT_DTYPE = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
@@ -262,6 +263,29 @@ def l0_ntw(sorted_hits: np.ndarray, seg_offsets, multiplicity: int, window_ps: i
     d_l0 = torch.zeros(max(n, 1), dtype=torch.uint8, device="cuda")
     d_ns = torch.zeros(1, dtype=torch.int32, device="cuda")
     tt_l0_ntw(d_sorted, seg, multiplicity, window_ps, d_l0, d_ns)
+    torch.cuda.synchronize()
+    return d_l0[:n].cpu().numpy(), int(d_ns.cpu().numpy().view(np.uint32)[0])
+
+
+def tt_l0_dntw(d_sorted: torch.Tensor, seg: Offsets, multiplicity: int, window_ps: int, d_l0: torch.Tensor,
+               d_n_start: torch.Tensor | None = None) -> None:
+    """Enqueue tt_l0_dntw (distinct-PMT level-0 trigger) on the current stream."""
+    _need_cuda()
+    n = d_sorted.shape[0]
+    assert d_l0.dtype == torch.uint8 and d_l0.numel() >= n
+    _check(load().tt_l0_dntw(_dp(d_sorted), c_u32(n), _dp(seg.d), c_u32(seg.count), c_u32(int(multiplicity)),
+                             ctypes.c_int64(int(window_ps)), _dp(d_l0), _dp(d_n_start), _stream()), "tt_l0_dntw")
+
+
+def l0_dntw(sorted_hits: np.ndarray, seg_offsets, multiplicity: int, window_ps: int):
+    """Host-array convenience around tt_l0_dntw -> (l0 bytes [n], number of firing starts)."""
+    _need_cuda()
+    d_sorted = hits_to_device(sorted_hits)
+    seg = Offsets(seg_offsets)
+    n = d_sorted.shape[0]
+    d_l0 = torch.full((max(n, 1),), 0xEE, dtype=torch.uint8, device="cuda")  # the call zeroes it itself
+    d_ns = torch.zeros(1, dtype=torch.int32, device="cuda")
+    tt_l0_dntw(d_sorted, seg, multiplicity, window_ps, d_l0, d_ns)
     torch.cuda.synchronize()
     return d_l0[:n].cpu().numpy(), int(d_ns.cpu().numpy().view(np.uint32)[0])
 
