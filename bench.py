@@ -344,7 +344,15 @@ def run_ours(args):
         l0["combine"] = {"kernel": "l0_combine_kernel", "ms": cb_ms, "alg_bytes_per_hit": 3,
                          "achieved": 3.0 * n / (cb_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                          "frac": 3.0 * n / (cb_ms * 1e-3) / 1e9 / peak, "n_cand_a": int(nc[0]), "n_cand_b": int(nc[1])}
-        del d_l0, d_pb, d_cd
+        # distinct-PMT variant DN7: 16 B read + 1 B zeroed + 1 B written per hit
+        d_dn = torch.empty(n, dtype=torch.uint8, device="cuda")
+        d_dnn = torch.zeros(1, dtype=torch.int32, device="cuda")
+        dn_ms = timed(lambda: B.tt_l0_dntw(d_out, seg, l0_n, l0_tw, d_dn, d_dnn), reps)
+        l0["dn"] = {"kernel": "l0_dntw_kernel", "multiplicity": l0_n, "window_ps": l0_tw, "ms": dn_ms,
+                    "alg_bytes_per_hit": 18, "achieved": 18.0 * n / (dn_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                    "frac": 18.0 * n / (dn_ms * 1e-3) / 1e9 / peak,
+                    "n_start": int(d_dnn.cpu().numpy().view(np.uint32)[0])}
+        del d_l0, d_pb, d_cd, d_dn
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
     e2e = None

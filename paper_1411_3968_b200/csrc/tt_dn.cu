@@ -7,7 +7,7 @@
 //   different PMT appears.
 //
 // One CTA per tile of kDTile sorted hits; the tile and kDHalo hits behind it are staged as (64-bit key, pmt).  Every
-// in-tile hit scans forward, keeping the different PMTs seen so far in registers (N <= 16); a window still open at the
+// in-tile hit scans forward, keeping the different PMTs seen so far (N <= 16) behind a Bloom mask; a window still open at the
 // staged end goes on in global memory, so the result is the plain definition for any density.  Members can lie in later
 // tiles: the output is zeroed by the call and every byte reaches it through atomicOr.
 #include "tt_common.cuh"
@@ -24,6 +24,7 @@ struct DnSmem {
     uint64_t key[kDStage];
     uint16_t pmt[kDStage];
     uint32_t f[kDTile / 4];  // result bytes of the tile
+    uint16_t seen[TT_MAX_DN_MULTIPLICITY][kDThreads];  // the different PMTs of the running window, one column per thread
     uint32_t red[kDThreads / 32];
 };
 
@@ -33,23 +34,6 @@ __device__ __forceinline__ void or_byte(uint8_t* base, uint32_t i, uint32_t bits
     const uintptr_t a = (uintptr_t)(base + i);
     atomicOr(reinterpret_cast<uint32_t*>(a & ~(uintptr_t)3), bits << (8 * (uint32_t)(a & 3)));
 }
-
-// the different PMTs seen so far, in registers; returns true when p was new
-struct PmtSet {
-    uint32_t v[TT_MAX_DN_MULTIPLICITY];
-    uint32_t cnt;
-    __device__ __forceinline__ bool add(uint32_t p) {
-        bool seen = false;
-#pragma unroll
-        for (int q = 0; q < TT_MAX_DN_MULTIPLICITY; ++q) seen |= (uint32_t)q < cnt && v[q] == p;
-        if (seen) return false;
-#pragma unroll
-        for (int q = 0; q < TT_MAX_DN_MULTIPLICITY; ++q)
-            if ((uint32_t)q == cnt) v[q] = p;
-        ++cnt;
-        return true;
-    }
-};
 
 __global__ void __launch_bounds__(kDThreads) l0_dntw_kernel(const uint4* __restrict__ hits, uint32_t n,
                                                             const uint32_t* __restrict__ seg_off, uint32_t n_seg,
@@ -91,20 +75,35 @@ __global__ void __launch_bounds__(kDThreads) l0_dntw_kernel(const uint4* __restr
         uint32_t sb = seg_b;
         if (!one_seg) sb = __ldg(seg_off + find_segment(seg_off, n_seg, k) + 1);
         const uint64_t tk = sm.key[q];
-        PmtSet set;
-        set.cnt = 0;
+        // N different PMTs need N hits: the plain N-in-TW test on hit k + N - 1 (staged: N - 1 < kDHalo) rules out most
+        // starts of a quiet tower before any scan
+        if ((uint64_t)k + N - 1 >= sb || sm.key[q + N - 1] - tk >= tw) continue;
+        // the different PMTs seen so far: a 64-bit Bloom mask in a register decides "new" in the common case, the exact
+        // list (a column of shared memory) is only read when the mask bit is already set
+        uint64_t mask = 0;
+        uint32_t cnt = 0;
+        auto add = [&](uint32_t p) -> bool {
+            const uint64_t bit = 1ull << (p & 63u);
+            if (mask & bit)
+                for (uint32_t c = 0; c < cnt; ++c)
+                    if (sm.seen[c][tid] == (uint16_t)p) return false;
+            mask |= bit;
+            sm.seen[cnt][tid] = (uint16_t)p;
+            ++cnt;
+            return true;
+        };
         bool fire = false, closed = false;
         uint32_t j = k;
         const uint32_t stage_end = min(sb, ghi);
         for (; j < stage_end; ++j) {  // the staged part of the window
             if (sm.key[j - tb] - tk >= tw) { closed = true; break; }
-            if (set.add(sm.pmt[j - tb]) && set.cnt == N) { fire = true; break; }
+            if (add(sm.pmt[j - tb]) && cnt == N) { fire = true; break; }
         }
         if (!fire && !closed) {       // still open at the staged end: on in global memory
             for (; j < sb; ++j) {
                 const uint4 v = __ldg(hits + j);
                 if (key_of(hit_time(v)) - tk >= tw) break;
-                if (set.add(v.z & 0xFFFFu) && set.cnt == N) { fire = true; break; }
+                if (add(v.z & 0xFFFFu) && cnt == N) { fire = true; break; }
             }
         }
         if (!fire) continue;
