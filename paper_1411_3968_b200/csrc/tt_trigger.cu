@@ -539,6 +539,49 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
 // rows of a tile of hits and of everything their masks can name (+-(kRowSpan - 1) list positions) are
 // staged in shared memory, so a neighbour's row is a shared-memory read at a word offset.
 constexpr int kClqTile = 256;
+
+// The same depth-first search as the generic loop in l2_clique_kernel (lowest candidate first, remove it, descend
+// with cand & adj(v) while enough candidates are left), written as a recursion over the number REM of vertices still
+// wanted so that every candidate mask is a statically indexed register array: NW words cover the frame of x, and
+// the depth is a template parameter.  Returns 0 = no clique, 1 = found, 2 = a wide row was met (slow list).
+template <int NW, int REM>
+struct CliqueDfs {
+    static __device__ __forceinline__ int run(uint32_t (&c)[NW], int cnt, uint32_t fx, const Row* s_rows, uint32_t base) {
+        while (cnt >= REM) {
+            uint32_t v = 0;
+            bool got = false;
+#pragma unroll
+            for (int i = 0; i < NW; ++i)
+                if (!got && c[i]) { v = 32u * (uint32_t)i + (uint32_t)__ffs(c[i]) - 1u; got = true; }
+#pragma unroll
+            for (int i = 0; i < NW; ++i)
+                if ((uint32_t)i == (v >> 5)) c[i] &= ~(1u << (v & 31u));
+            --cnt;
+            if (REM == 1) return 1;  // v completes the clique
+            const Row& rv = s_rows[32u * fx + v - base];
+            if (rv.f == kWide) return 2;
+            const int off = (int)fx - (int)rv.f;  // word i of x's frame is word i + off of v's
+            uint32_t nx[NW];
+            int cn = 0;
+#pragma unroll
+            for (int i = 0; i < NW; ++i) {
+                const int j = i + off;
+                const uint32_t a = (j >= 0 && j < kRowWords) ? rv.w[j] : 0u;
+                nx[i] = c[i] & a;
+                cn += __popc(nx[i]);
+            }
+            if (cn >= REM - 1) {
+                const int r = CliqueDfs<NW, REM - 1>::run(nx, cn, fx, s_rows, base);
+                if (r) return r;
+            }
+        }
+        return 0;
+    }
+};
+template <int NW>
+struct CliqueDfs<NW, 0> {
+    static __device__ __forceinline__ int run(uint32_t (&)[NW], int, uint32_t, const Row*, uint32_t) { return 1; }
+};
 constexpr int kClqStage = kClqTile + 2 * (kRowSpan - 1);  // 766 rows, 36.8 KB
 
 __global__ void __launch_bounds__(kClqTile) l2_clique_kernel(const L1Rec* __restrict__ l1, const uint32_t* __restrict__ m_ptr,
@@ -575,7 +618,23 @@ __global__ void __launch_bounds__(kClqTile) l2_clique_kernel(const L1Rec* __rest
         const uint32_t x = x0 + tid;
         if (x < x1) {
             const Row& rx = s_rows[x - base];
-            if (rx.f != kWide && (rx.deg & 0xFFFFu) + 1 >= N) {
+            if (rx.f != kWide && (rx.deg & 0xFFFFu) + 1 >= N && (rx.deg >> 16) <= 3u && K <= 4) {
+                // the usual case (a window of <= 96 candidates, N <= 5): masks in registers
+                uint32_t c0[3] = {rx.w[0], rx.w[1], rx.w[2]};
+                const int cnt0 = (int)(rx.deg & 0xFFFFu);
+                int r = 0;
+                switch (K) {
+                    case 2: r = CliqueDfs<3, 2>::run(c0, cnt0, rx.f, s_rows, base); break;
+                    case 3: r = CliqueDfs<3, 3>::run(c0, cnt0, rx.f, s_rows, base); break;
+                    default: r = CliqueDfs<3, 4>::run(c0, cnt0, rx.f, s_rows, base); break;
+                }
+                if (r == 2) {
+                    slow_list[atomicAdd(slow_cnt, 1u)] = x;
+                } else if (r == 1) {
+                    flags[l1[x].idx] |= (uint8_t)TT_L2;
+                    l2bit[x] = 1;
+                }
+            } else if (rx.f != kWide && (rx.deg & 0xFFFFu) + 1 >= N) {
                 uint32_t cand[TT_MAX_MULTIPLICITY][kRowWords];
                 const int nw = (int)(rx.deg >> 16);  // words of the frame that can hold a neighbour of x
                 for (int i = 0; i < nw; ++i) cand[0][i] = rx.w[i];
