@@ -245,20 +245,52 @@ def run_ours(args):
     l1_frac = float((d_flags & 4).ne(0).float().mean().item())
     inevt_frac = float((d_flags & 32).ne(0).float().mean().item())
 
+    # The step (24 launches + 3 memsets) is captured once in a CUDA graph and replayed in the timed region: the library
+    # allocates nothing and never synchronises in its hot calls.  Launch gaps are most of cfg0 / cfg1 (0.22 -> 0.09 ms,
+    # 0.24 -> 0.11 ms) and still ~0.1 ms of the large configs.  The per-stage events cannot be recorded inside a replay:
+    # they come from a separate, untimed, profiled pass of direct launches.
+    use_graph = args.graph in ("on", "auto")
+    graph, graph_note, launches_per_replay = None, None, 0
+    if use_graph:
+        try:
+            cg = torch.cuda.CUDAGraph()
+            lc = B.launch_count()
+            with torch.cuda.graph(cg):
+                step()
+            launches_per_replay = B.launch_count() - lc
+            cg.replay()
+            torch.cuda.synchronize()
+            chk = d_cnt.cpu().numpy().view(np.uint32)
+            assert (int(chk[0]), int(chk[1]), int(chk[2])) == (n_seeds, n_events, status), "graph replay differs"
+            graph = cg
+        except Exception as ex:  # capture not possible here: time the direct launches
+            graph, graph_note = None, f"capture failed: {type(ex).__name__}"
+            torch.cuda.synchronize()
+    run = graph.replay if graph is not None else step
+
     sampler = ClockSampler(local)
-    B.prof_enable(True)
+    if graph is None:
+        B.prof_enable(True)
     l0 = B.launch_count()
     barrier()
     sampler.start()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     for _ in range(args.steps):
-        step()
+        run()
     e1.record()
     barrier()
     clocks = sampler.stop()
-    launches = B.launch_count() - l0
+    launches = B.launch_count() - l0 if graph is None else launches_per_replay * args.steps
     ms_total = e0.elapsed_time(e1)
+    if graph is not None:  # stage breakdown from direct launches, outside the timed region
+        B.prof_enable(True)
+        step()             # first profiled step creates the event pool and the pinned counter buffers: not measured
+        barrier()
+        B.prof_enable(True)  # clears the marks
+        for _ in range(args.steps):
+            step()
+        barrier()
     stages = B.prof_read()
     B.prof_enable(False)
     ms_step = ms_total / args.steps
@@ -409,7 +441,8 @@ def run_ours(args):
                        "ms_per_200ms_slice": ms_step / slices, "l2_flush": "inputs larger than L2 (16 B x n)"
                        if 16 * n > 130e6 else "inputs fit in L2: not flushed (launch-bound config)",
                        "n_seeds": n_seeds, "n_events": n_events, "status": status, "l1_fraction": l1_frac,
-                       "inevt_fraction": inevt_frac, "parallelism": f"slice-per-gpu x{world}"},
+                       "inevt_fraction": inevt_frac, "parallelism": f"slice-per-gpu x{world}",
+                       "cuda_graph": graph is not None, "cuda_graph_note": graph_note},
             "clocks": clocks, "gpu_launches": int(launches),
             "roofline": roof,
             "pipeline_roofline": {"alg_bytes_per_hit": ALG_BYTES_PIPELINE, "achieved": pipe_ach, "peak": peak,
@@ -432,6 +465,8 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--scale", type=float, default=1.0, help="time_scale < 1 shrinks the workload (debugging only)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
+                    help="replay the step as a CUDA graph in the timed region (auto: yes, direct launches if capture fails)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

@@ -43,10 +43,17 @@ struct Counter {
     uint32_t* host;  // pinned
 };
 static std::vector<Counter> g_counters;
+// pinned slots are pooled and reused from one profiled pass to the next: cudaMallocHost is a slow, synchronous host call,
+// and one per sample showed up as device idle time in whatever stage was open (bench.py, small configs)
+static std::vector<uint32_t*> g_pinned;
 void prof_counter(cudaStream_t s, const char* name, const uint32_t* d_value) {
     if (!g_on || g_counters.size() >= 4096) return;
-    uint32_t* h = nullptr;
-    if (cudaMallocHost(&h, sizeof(uint32_t)) != cudaSuccess) return;
+    if (g_counters.size() == g_pinned.size()) {
+        uint32_t* h = nullptr;
+        if (cudaMallocHost(&h, sizeof(uint32_t)) != cudaSuccess) return;
+        g_pinned.push_back(h);
+    }
+    uint32_t* h = g_pinned[g_counters.size()];
     *h = 0;
     cudaMemcpyAsync(h, d_value, sizeof(uint32_t), cudaMemcpyDeviceToHost, s);
     g_counters.push_back({name, h});
@@ -60,8 +67,7 @@ extern "C" int tt_prof_enable(int on) {
     tt::g_on = on != 0;
     tt::g_marks.clear();
     tt::g_used = 0;
-    for (auto& c : tt::g_counters) cudaFreeHost(c.host);
-    tt::g_counters.clear();
+    tt::g_counters.clear();  // the pinned slots stay in the pool
     return TT_OK;
 }
 
