@@ -357,3 +357,49 @@ def test_reused_dirty_workspaces_and_determinism(cfg, ts, ss, B, oracle_lib):
         ev = d_ev[:ne].cpu().numpy().reshape(-1).view(B.EVENT_DTYPE)
         assert ne == len(o["events"]) and ev.tobytes() == o["events"].tobytes(), it
     geo.close()
+
+
+@pytest.mark.parametrize("cfg,ts,ss", [(1, 0.1, 1), (4, 0.002, 1)])
+def test_cuda_graph_replay(cfg, ts, ss, B, oracle_lib):
+    """bench.py replays the step as a CUDA graph: the three calls allocate nothing and never synchronise, so they can be
+    captured as they are.  Replays onto garbage-filled outputs and workspaces give the oracle's bytes every time."""
+    w = W.make_config(cfg, time_scale=ts, seg_scale=ss)
+    p = w.params
+    o = oracle_chain(w.hits, w.seg_offsets, w.geometry, p)
+    n = w.n
+    geo, prm = _geo(B, w.geometry), _prm(B, p)
+    seg, runs = B.Offsets(w.seg_offsets), B.Offsets(w.run_offsets)
+    d_in = B.hits_to_device(w.hits)
+    d_out = torch.empty_like(d_in)
+    d_flags = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    d_seeds = torch.zeros(n, dtype=torch.int32, device="cuda")
+    d_ev = torch.zeros((n, 4), dtype=torch.int64, device="cuda")
+    d_cnt = torch.zeros(4, dtype=torch.int32, device="cuda")
+    ws = {}
+
+    def step():
+        d_cnt.zero_()
+        ws["s"] = B.tt_sort_slice(d_in, d_out, None, seg, runs, d_cnt[2:3], ws.get("s"))
+        ws["t"] = B.tt_trigger_slice(d_out, seg, geo, prm, d_flags, d_seeds, d_cnt[0:1], d_cnt[2:3], ws.get("t"))
+        ws["e"] = B.tt_extract_events(d_out, seg, d_seeds, d_cnt[0:1], prm, d_ev, d_cnt[1:2], d_flags, None, None,
+                                      d_cnt[2:3], ws.get("e"))
+
+    step()  # workspaces allocated, kernel attributes set: outside the capture
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        step()
+    for it in range(3):
+        for t in (d_out, d_flags, d_seeds, d_ev, d_cnt, ws["s"], ws["t"], ws["e"]):
+            t.fill_(-1 if t.dtype in (torch.int32, torch.int64) else 0xA5)
+        g.replay()
+        torch.cuda.synchronize()
+        cnt = d_cnt.cpu().numpy().view(np.uint32)
+        ns, ne, status = int(cnt[0]), int(cnt[1]), int(cnt[2])
+        assert status == 0, it
+        assert B.hits_to_host(d_out).tobytes() == o["sorted"].tobytes(), it
+        assert (d_flags.cpu().numpy() == o["flags"]).all(), it
+        assert ns == len(o["seeds"]) and (d_seeds[:ns].cpu().numpy().view(np.uint32) == o["seeds"]).all(), it
+        ev = d_ev[:ne].cpu().numpy().reshape(-1).view(B.EVENT_DTYPE)
+        assert ne == len(o["events"]) and ev.tobytes() == o["events"].tobytes(), it
+    geo.close()
