@@ -15,12 +15,12 @@
 
 namespace tt {
 
-constexpr int kL0Threads = 256;
+constexpr int kL0Threads = 128;
 constexpr int kL0Per = 8;
-constexpr int kL0Tile = kL0Threads * kL0Per;   // 2048
+constexpr int kL0Tile = kL0Threads * kL0Per;   // 1024
 static_assert(TT_MAX_L0_MULTIPLICITY - 1 <= 256, "the wide halo covers the longest window");
 
-// kHalo staged hits before and after the tile (>= N - 1, multiple of 32): 32 for N <= 33 (N7TW: 3 % of re-reads, 17 KB
+// kHalo staged hits before and after the tile (>= N - 1, multiple of 32): 32 for N <= 33 (N7TW: 6 % of re-reads, 10 KB
 // of shared memory per CTA), 256 for the long windows.  Small CTAs on purpose: the kernel is bound by the latency of
 // its staging loads, so what counts is how many CTAs are resident per SM (ncu, profiles/r1_v6.md).
 template <int kHalo>
@@ -32,7 +32,7 @@ struct L0Smem {
 };
 
 template <int kHalo>
-__global__ void __launch_bounds__(kL0Threads, 8) l0_ntw_kernel(const uint4* __restrict__ hits, uint32_t n,
+__global__ void __launch_bounds__(kL0Threads, 16) l0_ntw_kernel(const uint4* __restrict__ hits, uint32_t n,
                                                                const uint32_t* __restrict__ seg_off, uint32_t n_seg,
                                                                uint32_t N, uint64_t tw, uint8_t* __restrict__ l0,
                                                                uint32_t* __restrict__ n_start) {
