@@ -80,6 +80,10 @@ int64_t dtmax(const Geo& g, uint32_t a, uint32_t b) {
     return g.blocks[((size_t)blk * g.ppt + (a % g.ppt)) * g.ppt + (b % g.ppt)];
 }
 
+// Exact t_hi - t_lo for t_hi >= t_lo (hits are time-sorted where this is used).  DESIGN.md reading R1: timestamps are
+// "any int64", so a span can reach 2^64 - 1 and does not fit int64; it always fits uint64.
+uint64_t span(int64_t t_hi, int64_t t_lo) { return (uint64_t)t_hi - (uint64_t)t_lo; }
+
 // Is there a subset of `need` members of cand[from..], pairwise adjacent?  Plain recursion.
 bool has_clique(const std::vector<std::vector<uint8_t>>& adj, const std::vector<int>& cand, int need) {
     if (need == 0) return true;
@@ -119,7 +123,7 @@ int oracle_trigger(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n
                    const Params* p, uint8_t* flags, uint32_t* seeds, uint32_t* n_seeds, int32_t* status) {
     if (p->l2_multiplicity < 1 || p->lc_window_ps < 0 || p->l2_window_ps < 0) return -1;
     const Geo g{n_pmt, n_tower, ppt, pair_block, blocks};
-    const int64_t LC = p->lc_window_ps, W = p->l2_window_ps;
+    const uint64_t LC = (uint64_t)p->lc_window_ps, W = (uint64_t)p->l2_window_ps;
     const int N = (int)p->l2_multiplicity;
     *status = 0;
     std::memset(flags, 0, n);
@@ -131,9 +135,9 @@ int oracle_trigger(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n
             uint8_t f = 0;
             if (h[i].charge >= p->q_thresh) f |= F_Q;
             bool lc = false;
-            for (int64_t j = i - 1; j >= a && h[i].t_ps - h[j].t_ps <= LC; --j)
+            for (int64_t j = i - 1; j >= a && span(h[i].t_ps, h[j].t_ps) <= LC; --j)
                 if (h[j].floor == h[i].floor && h[j].pmt_id != h[i].pmt_id) lc = true;
-            for (int64_t j = i + 1; j < b && h[j].t_ps - h[i].t_ps <= LC; ++j)
+            for (int64_t j = i + 1; j < b && span(h[j].t_ps, h[i].t_ps) <= LC; ++j)
                 if (h[j].floor == h[i].floor && h[j].pmt_id != h[i].pmt_id) lc = true;
             if (lc) f |= F_LC;
             if (f) f |= F_L1;
@@ -149,15 +153,17 @@ int oracle_trigger(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n
         const int64_t m = (int64_t)l1.size();
         auto edge = [&](int64_t x, int64_t y) {  // x, y index l1[]
             const Hit &hx = h[l1[x]], &hy = h[l1[y]];
-            const int64_t d = hx.t_ps > hy.t_ps ? hx.t_ps - hy.t_ps : hy.t_ps - hx.t_ps;
-            const int64_t lim = std::min<int64_t>(dtmax(g, hx.pmt_id, hy.pmt_id), W);
-            return lim >= 0 && d <= lim;
+            const uint64_t d = hx.t_ps > hy.t_ps ? span(hx.t_ps, hy.t_ps) : span(hy.t_ps, hx.t_ps);
+            const int64_t tab = dtmax(g, hx.pmt_id, hy.pmt_id);
+            if (tab < 0) return false;
+            const uint64_t lim = std::min<uint64_t>((uint64_t)tab, W);
+            return d <= lim;
         };
         for (int64_t x = 0; x < m; ++x) {
             std::vector<int64_t> nb;  // neighbours of x, ascending
             int64_t lo = x;
-            while (lo > 0 && h[l1[x]].t_ps - h[l1[lo - 1]].t_ps <= W) --lo;
-            for (int64_t y = lo; y < m && h[l1[y]].t_ps - h[l1[x]].t_ps <= W; ++y)
+            while (lo > 0 && span(h[l1[x]].t_ps, h[l1[lo - 1]].t_ps) <= W) --lo;
+            for (int64_t y = lo; y < m && (y <= x || span(h[l1[y]].t_ps, h[l1[x]].t_ps) <= W); ++y)
                 if (y != x && edge(x, y)) nb.push_back(y);
             const int k = (int)nb.size();
             if (k < N - 1) continue;
@@ -195,14 +201,17 @@ int oracle_events(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n_
         while (k < n_seeds && seeds[k] < b) {
             uint32_t first = k, last = k;
             while (last + 1 < n_seeds && seeds[last + 1] < b &&
-                   h[seeds[last + 1]].t_ps - h[seeds[last]].t_ps <= 2 * H)
+                   span(h[seeds[last + 1]].t_ps, h[seeds[last]].t_ps) <= 2 * (uint64_t)H)
                 ++last;
+            // window bounds in exact arithmetic (R1: any int64 timestamp); the reported int64 fields are the exact
+            // values where they fit, else modulo 2^64 (R13: unclipped)
+            const __int128 ts = (__int128)h[seeds[first]].t_ps - H, te = (__int128)h[seeds[last]].t_ps + H;
             Event e;
-            e.t_start = h[seeds[first]].t_ps - H;
-            e.t_end = h[seeds[last]].t_ps + H;
+            e.t_start = (int64_t)(uint64_t)ts;
+            e.t_end = (int64_t)(uint64_t)te;
             uint32_t lo = seeds[first], hi = seeds[last] + 1;
-            while (lo > a && h[lo - 1].t_ps >= e.t_start) --lo;  // lower_bound(t >= t_start)
-            while (hi < b && h[hi].t_ps <= e.t_end) ++hi;        // upper_bound(t <= t_end)
+            while (lo > a && (__int128)h[lo - 1].t_ps >= ts) --lo;  // lower_bound(t >= t_start)
+            while (hi < b && (__int128)h[hi].t_ps <= te) ++hi;      // upper_bound(t <= t_end)
             e.hit_begin = lo;
             e.hit_end = hi;
             e.seed_begin = first;

@@ -106,7 +106,9 @@ __global__ void __launch_bounds__(1024) merge_setup_kernel(LevelDev lv, const ui
             const uint32_t n_g = lv.roff[r1] - lv.roff[r0];
             const uint32_t nt = tiles_for(n_g);
             lv.gT0[g] = kmin;
-            lv.gDT[g] = nt ? (kmax >= kmin ? (kmax - kmin) / nt + 1 : 1) : 1;
+            uint64_t dt = nt ? (kmax >= kmin ? (kmax - kmin) / nt + 1 : 1) : 1;
+            if (dt == 0) dt = ~0ull;  // one tile over the whole key range, 2^64 - 1: the + 1 wrapped
+            lv.gDT[g] = dt;
             lv.roff_next[g] = lv.roff[r0];
         }
     }

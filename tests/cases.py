@@ -155,6 +155,31 @@ def directed_cases():
                     seeds=[0, 1, 2, 3],
                     events=[(-big - H, -big + 15_000 + H, 0, 2, 0, 2), (big - H, big + 10 + H, 2, 4, 2, 2)])))
 
+    # --- R1: a span of 2^63 ps between two clusters: t_hi - t_lo does not fit int64 (unsigned differences) ----
+    big2 = 1 << 62
+    cs.append(dict(
+        name="span_2_63_between_clusters",
+        rows=[(big2 + 10, 1, 0, 400), (-big2, 0, 0, 400), (big2, 0, 0, 400), (-big2 + 15_000, 1, 0, 100)],
+        seg=[0, 4], table=_table(4), params=dict(l2_multiplicity=2),
+        expect=dict(order=[1, 3, 2, 0],
+                    flags=[Q | LC | L1 | STAR | L2 | EV, LC | L1 | STAR | L2 | EV, Q | LC | L1 | STAR | L2 | EV,
+                           Q | LC | L1 | STAR | L2 | EV],
+                    seeds=[0, 1, 2, 3],
+                    events=[(-big2 - H, -big2 + 15_000 + H, 0, 2, 0, 2), (big2 - H, big2 + 10 + H, 2, 4, 2, 2)])))
+
+    # --- R1 / R13: hits at both ends of int64: the span is 2^64 - 1, and t_start / t_end (unclipped) leave int64 --
+    # reported modulo 2^64, while the hit ranges follow the exact (unwrapped) window
+    lo64, hi64 = -(1 << 63), (1 << 63) - 1
+    cs.append(dict(
+        name="int64_extremes_windows_wrap",
+        rows=[(hi64, 1, 1, 400), (lo64, 0, 0, 400), (hi64 - 10, 0, 0, 400), (lo64 + 10, 1, 1, 400)],
+        seg=[0, 4], table=_table(4), params=dict(l2_multiplicity=2),
+        expect=dict(order=[1, 3, 2, 0],
+                    flags=[Q | L1 | STAR | L2 | EV] * 4,
+                    seeds=[0, 1, 2, 3],
+                    events=[(lo64 - H + (1 << 64), lo64 + 10 + H, 0, 2, 0, 2),
+                            (hi64 - 10 - H, hi64 + H - (1 << 64), 2, 4, 2, 2)])))
+
     # --- R9: the window binds before the table ----------------------------------------------------
     cs.append(dict(
         name="l2_window_binds",
