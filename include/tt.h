@@ -77,9 +77,9 @@ enum {
     TT_S_RUN_UNSORTED = 4,   /* a run given by d_run_offsets is not non-decreasing: output unspecified */
     TT_S_BAD_PMT = 8,        /* an L1 hit has pmt_id >= n_pmt (it has no L2 edges)                     */
     TT_S_DENSITY = 16        /* an L1 hit has more than TT_MAX_NEIGHBOURS L1 hits of its segment within
-                                +-min(W, largest table entry) of it: its L2STAR bit is exact, its
-                                clique-mode L2 bit is not decided (left clear unless another hit's
-                                clique contains it)                                                  */
+                                +-min(W, largest table entry) of it: its L2STAR bit is exact, and its
+                                clique-mode L2 bit is SET FROM the L2STAR bit (fail open: a superset of
+                                the exact answer, the same on every run; the hit stays in the data)  */
 };
 #define TT_MAX_MULTIPLICITY 16
 #define TT_MAX_NEIGHBOURS 2048

@@ -762,9 +762,15 @@ __global__ void __launch_bounds__(kL2Warps * 32) l2_wide_kernel(const L1Rec* __r
         bool l2 = star;
         if (star && mode == 0 && N > 2) {
             l2 = false;
+            // lane 0 reads the byte another warp may be writing and shares it: the full-mask votes and shuffles of the
+            // search below need every lane of the warp on the same path
+            const uint32_t marked = __shfl_sync(0xffffffffu, lane == 0 ? (uint32_t)l2bit[x] : 0u, 0);
             if (!fits) {
+                // more than TT_MAX_NEIGHBOURS candidates: the clique is not searched.  Fail open and deterministic: the
+                // hit keeps its data (L2 := the exact L2STAR bit, a superset of the clique answer) and the status says so
                 if (lane == 0) atomicOr(status, TT_S_DENSITY);
-            } else if (l2bit[x]) {
+                l2 = true;
+            } else if (marked) {
                 l2 = true;  // already marked as a member of a clique found from another hit
             } else {
                 // need K vertices of mask[0], pairwise adjacent

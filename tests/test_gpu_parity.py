@@ -137,6 +137,15 @@ def test_status_codes(B, oracle_lib):
     r = B.process_slice(w.hits, w.seg_offsets, w.run_offsets, geo, prm, seed_cap=3, event_cap=1)
     assert r.status & B.TT_S_SEED_OVERFLOW and r.n_seeds == len(o["seeds"]) and (r.seeds == o["seeds"][:3]).all()
     assert (r.flags & 31 == o["flags"] & 31).all()
+    # event capacity alone too small: the true count, the first event_cap events, every flag (INEVT included)
+    w2 = W.make_config(1, time_scale=0.2)
+    o2 = oracle_chain(w2.hits, w2.seg_offsets, w2.geometry, w2.params)
+    assert len(o2["events"]) > 2
+    r = B.process_slice(w2.hits, w2.seg_offsets, w2.run_offsets, geo, prm, event_cap=2)
+    assert r.status == B.TT_S_EVENT_OVERFLOW
+    assert r.n_events == len(o2["events"]) and r.events.tobytes() == o2["events"][:2].tobytes()
+    assert r.n_seeds == len(o2["seeds"]) and (r.seeds == o2["seeds"]).all()
+    assert (r.flags & 31 == o2["flags"] & 31).all()
     # an unsorted run
     h = w.hits.copy()
     a = int(w.run_offsets[3])
@@ -177,9 +186,16 @@ def test_dense_neighbourhood(B, oracle_lib):
         r = B.process_slice(h, seg, None, geo, _prm(B, p))
         assert ((r.flags & 8) == (o["flags"] & 8)).all()
         if expect_density:
-            assert r.status & B.TT_S_DENSITY
+            # fail open (R10): the dense hits get L2 := L2STAR, the status says so, and nothing else changes --
+            # the 200 isolated hits (> 1 s away: no coincidence or event reaches them) are the oracle's clique-mode bytes
+            assert r.status == B.TT_S_DENSITY
             dense = np.arange(len(h)) < m
-            assert not (r.flags & 16)[dense].any()
+            assert (((r.flags & 16) != 0)[dense] == ((r.flags & 8) != 0)[dense]).all() and (r.flags & 16)[dense].all()
+            iso = oracle_chain(h[m:], np.array([0, 200], dtype=np.uint32), geo_w, p)
+            assert (r.flags[m:] == iso["flags"]).all()
+            assert (r.seeds == np.concatenate([np.arange(m), iso["seeds"] + m])).all()
+            r2 = B.process_slice(h, seg, None, geo, _prm(B, p))  # the same bytes on every run
+            assert (r2.flags == r.flags).all() and (r2.seeds == r.seeds).all() and r2.events.tobytes() == r.events.tobytes()
         else:
             assert r.status == 0
             assert (r.flags == o["flags"]).all() and (r.seeds == o["seeds"]).all()
