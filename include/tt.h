@@ -20,6 +20,9 @@
  *   h_*   host pointers; `p`, `g`, `ws_bytes` are host pointers too
  *   All hot calls are asynchronous: they enqueue kernels on `stream` (a cudaStream_t passed as
  *   void*) and return.  The return value covers argument errors only (TT_OK / TT_E_*).
+ *   The library keeps no state between calls apart from per-device one-time kernel set-up and a per-host-thread copy
+ *   of the last merge plan (both invisible in the results); calls from several host threads and on several devices
+ *   are allowed.
  *   Data-dependent conditions are OR-ed into *d_status (device int32, zeroed by the caller or by
  *   a previous call's owner), to be read after synchronising: TT_S_* bits.
  *   Workspace: call with d_ws == NULL to get the required size in *ws_bytes (nothing is enqueued);
@@ -121,6 +124,20 @@ int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_o
                      const uint32_t* h_seg_offsets, uint32_t n_seg, const tt_geometry* g,
                      const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds, uint32_t seed_cap,
                      uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes, int32_t* d_status, void* stream);
+
+/* tt_sort_slice followed by tt_trigger_slice as ONE call (last bullet):
+ * the same arguments, the same outputs byte for byte (d_out, d_perm, d_flags, d_seeds, *d_n_seeds, status bits).
+ * With runs given, the L1 step (Q | same-floor coincidence) is evaluated by the last merge level on its time tile
+ * while the sorted tile is in shared memory, so the sorted array is not read a second time for it; the hits within
+ * lc_window of a tile edge are finished by exact scans afterwards (the paper's "edge" rule between sub-slices,
+ * PAPER.md:47).  Without runs it is the two calls back to back.  Workspace = both calls' workspaces; same alignment
+ * and error rules as the two calls. */
+int tt_sort_trigger_slice(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n,
+                          const uint32_t* d_seg_offsets, const uint32_t* h_seg_offsets, uint32_t n_seg,
+                          const uint32_t* d_run_offsets, const uint32_t* h_run_offsets, uint32_t n_runs,
+                          const tt_geometry* g, const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds,
+                          uint32_t seed_cap, uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes, int32_t* d_status,
+                          void* stream);
 
 /* Merge the closed windows [t-H, t+H] of consecutive seeds (merge <=> gap <= 2H, never across a
  * segment) into d_events[event_cap]; *d_n_events = true count.  The seed list is read from the

@@ -24,7 +24,7 @@ TT_S_SEED_OVERFLOW, TT_S_EVENT_OVERFLOW, TT_S_RUN_UNSORTED, TT_S_BAD_PMT, TT_S_D
 EXPORTS = ["tt_version", "tt_geometry_create", "tt_geometry_destroy", "tt_sort_slice", "tt_trigger_slice",
            "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host", "tt_launch_count",
            "tt_prof_enable", "tt_prof_read", "tt_l0_ntw", "tt_pair_seeds", "tt_l0_combine",
-           "tt_l0_dntw"]
+           "tt_l0_dntw", "tt_sort_trigger_slice"]
 
 HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
 EVENT_DTYPE = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
@@ -218,6 +218,30 @@ def tt_trigger_slice(d_sorted: torch.Tensor, seg: Offsets, geo: Geometry, params
     return ws
 
 
+def tt_sort_trigger_slice(d_in: torch.Tensor, d_out: torch.Tensor, d_perm: torch.Tensor | None, seg: Offsets,
+                          runs: Offsets | None, geo: Geometry, params: TTParams, d_flags: torch.Tensor,
+                          d_seeds: torch.Tensor, d_n_seeds: torch.Tensor, d_status: torch.Tensor,
+                          ws: torch.Tensor | None = None) -> torch.Tensor:
+    """Enqueue tt_sort_trigger_slice (tt_sort_slice + tt_trigger_slice in one call, L1 fused into the last merge
+    level) on the current stream.  Returns the workspace tensor used (reusable)."""
+    _need_cuda()
+    L = load()
+    n = d_in.shape[0]
+
+    def call(wsp, nbytes):
+        return L.tt_sort_trigger_slice(_dp(d_in), _dp(d_out), _dp(d_perm), c_u32(n), _dp(seg.d), _hp(seg.h),
+                                       c_u32(seg.count), _dp(runs.d) if runs else c_vp(0),
+                                       _hp(runs.h) if runs else c_vp(0), c_u32(runs.count if runs else 0), geo.handle,
+                                       ctypes.byref(params), _dp(d_flags), _dp(d_seeds), c_u32(d_seeds.numel()),
+                                       _dp(d_n_seeds), wsp, nbytes, _dp(d_status), _stream())
+
+    if ws is None:
+        ws = _ws(call, "tt_sort_trigger_slice")
+    nb = c_sz(ws.numel())
+    _check(call(_dp(ws), ctypes.byref(nb)), "tt_sort_trigger_slice")
+    return ws
+
+
 def tt_extract_events(d_sorted: torch.Tensor, seg: Offsets, d_seeds: torch.Tensor, d_n_seeds: torch.Tensor,
                       params: TTParams, d_events: torch.Tensor, d_n_events: torch.Tensor,
                       d_flags: torch.Tensor | None, d_gather: torch.Tensor | None, d_n_gathered: torch.Tensor | None,
@@ -347,8 +371,9 @@ class SliceResult:
 
 
 def process_slice(hits: np.ndarray, seg_offsets, run_offsets, geo: Geometry, params: TTParams, seed_cap=None,
-                  event_cap=None, gather=False) -> SliceResult:
-    """Convenience for tests: upload, run the three calls, download everything."""
+                  event_cap=None, gather=False, fused=False) -> SliceResult:
+    """Convenience for tests: upload, run the three calls (fused: tt_sort_trigger_slice + tt_extract_events),
+    download everything."""
     _need_cuda()
     n = len(hits)
     seg = Offsets(seg_offsets)
@@ -359,15 +384,18 @@ def process_slice(hits: np.ndarray, seg_offsets, run_offsets, geo: Geometry, par
     d_status = torch.zeros(1, dtype=torch.int32, device="cuda")
     seed_cap = n if seed_cap is None else seed_cap
     event_cap = n if event_cap is None else event_cap
-    d_flags = torch.zeros(max(n, 1), dtype=torch.uint8, device="cuda")
+    d_flags = torch.full((max(n, 1),), 0xEE if fused else 0, dtype=torch.uint8, device="cuda")  # every byte is written
     d_seeds = torch.zeros(max(seed_cap, 1), dtype=torch.int32, device="cuda")[:seed_cap]
     d_ns = torch.zeros(1, dtype=torch.int32, device="cuda")
     d_ev = torch.zeros((max(event_cap, 1), 4), dtype=torch.int64, device="cuda")[:event_cap]
     d_ne = torch.zeros(1, dtype=torch.int32, device="cuda")
     d_g = torch.zeros((max(n, 1), 2), dtype=torch.int64, device="cuda") if gather else None
     d_ng = torch.zeros(1, dtype=torch.int32, device="cuda") if gather else None
-    tt_sort_slice(d_in, d_out, d_perm, seg, runs, d_status)
-    tt_trigger_slice(d_out, seg, geo, params, d_flags, d_seeds, d_ns, d_status)
+    if fused:
+        tt_sort_trigger_slice(d_in, d_out, d_perm, seg, runs, geo, params, d_flags, d_seeds, d_ns, d_status)
+    else:
+        tt_sort_slice(d_in, d_out, d_perm, seg, runs, d_status)
+        tt_trigger_slice(d_out, seg, geo, params, d_flags, d_seeds, d_ns, d_status)
     tt_extract_events(d_out, seg, d_seeds, d_ns, params, d_ev, d_ne, d_flags, d_g, d_ng, d_status)
     torch.cuda.synchronize()
     ns, ne = int(d_ns.item()) & 0xFFFFFFFF, int(d_ne.item()) & 0xFFFFFFFF

@@ -3,17 +3,40 @@
 #include <cstring>
 #include <vector>
 
-#include "tt_common.cuh"
+#include <mutex>
+
+#include "tt_merge.cuh"
 
 namespace tt {
 size_t radix_ws_bytes(uint32_t n);
 int radix_sort(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, const uint32_t* d_seg_offsets,
                uint32_t n_seg, void* d_ws, cudaStream_t s);
-size_t merge_ws_bytes(uint32_t n, const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* h_run_offsets,
-                      uint32_t n_runs);
-int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, const uint32_t* d_seg_offsets,
-                    const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* d_run_offsets,
-                    const uint32_t* h_run_offsets, uint32_t n_runs, void* d_ws, int32_t* d_status, cudaStream_t s);
+
+constexpr int kMaxDev = 64;
+static std::mutex g_dev_mu;
+static uint32_t g_done[kMaxDev];
+static int g_sms[kMaxDev];
+
+int once_per_device(int slot, int (*fn)()) {
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess) return TT_E_CUDA;
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    if (d >= 0 && d < kMaxDev && ((g_done[d] >> slot) & 1u)) return TT_OK;
+    const int rc = fn();
+    if (rc == TT_OK && d >= 0 && d < kMaxDev) g_done[d] |= 1u << slot;
+    return rc;
+}
+
+int sm_count() {
+    int d = 0;
+    if (cudaGetDevice(&d) != cudaSuccess) return 148;
+    std::lock_guard<std::mutex> lk(g_dev_mu);
+    if (d >= 0 && d < kMaxDev && g_sms[d] > 0) return g_sms[d];
+    int v = 0;
+    if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, d) != cudaSuccess || v <= 0) v = 148;
+    if (d >= 0 && d < kMaxDev) g_sms[d] = v;
+    return v;
+}
 }  // namespace tt
 using namespace tt;
 
@@ -108,6 +131,6 @@ extern "C" int tt_sort_slice(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm
     cudaStream_t s = (cudaStream_t)stream;
     if (runs)
         return merge_sort_runs(d_in, d_out, d_perm, n, d_seg_offsets, h_seg_offsets, n_seg, d_run_offsets, h_run_offsets,
-                               n_runs, d_ws, d_status, s);
+                               n_runs, d_ws, d_status, s, nullptr, nullptr);
     return radix_sort(d_in, d_out, d_perm, n, d_seg_offsets, n_seg, d_ws, s);
 }

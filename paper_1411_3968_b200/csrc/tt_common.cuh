@@ -20,7 +20,11 @@
 
 namespace tt {
 
-constexpr int kSMs = 148;  // B200
+// Per-device one-time set-up (cudaFuncSetAttribute is per device): runs fn() once for (current device, slot), under a
+// lock, so a second GPU or a second host thread never launches before the attributes are set (tt_api.cu).
+enum { kSlotMerge = 0, kSlotTrigger = 1, kSlotPairs = 2 };
+int once_per_device(int slot, int (*fn)());
+int sm_count();  // SMs of the current device (cached per device)
 
 // ---- launch counter and stage profiler (tt_prof.cu) ------------------------------------------------
 void count_launch();                                // every kernel launch of the library goes through TT_K

@@ -336,7 +336,7 @@ extern "C" int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint3
     TT_K(ev_scan_kernel)<<<1, 1024, 0, s>>>(plan.cnt, kEvBlocks, d_n_events, event_cap, d_status);
     TT_K(ev_write_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(hits, d_seeds, d_n_seeds, seed_cap, sc, twoH, p->event_half_ps,
                                                      plan.cnt, plan.head, d_events, event_cap);
-    TT_K(ev_fix_kernel)<<<kSMs, 256, 0, s>>>(hits, sc, p->event_half_ps, d_events, d_n_events, event_cap);
+    TT_K(ev_fix_kernel)<<<(uint32_t)sm_count(), 256, 0, s>>>(hits, sc, p->event_half_ps, d_events, d_n_events, event_cap);
     if (d_gather || d_n_gathered) {
         prof_mark(s, "ev.gather_scan");
         TT_K(len_count_kernel)<<<kEvBlocks, kEvThreads, 0, s>>>(d_events, d_n_events, event_cap, plan.cnt2);

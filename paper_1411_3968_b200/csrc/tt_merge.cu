@@ -20,7 +20,9 @@
 #include <algorithm>
 #include <vector>
 
-#include "tt_common.cuh"
+#include <cstring>
+
+#include "tt_merge.cuh"
 
 namespace tt {
 
@@ -29,22 +31,8 @@ constexpr int kCap = 4096;                    // hits staged per chunk
 constexpr int kMItems = kCap / kMThreads;     // 8
 constexpr uint32_t kTileTarget = 3584;        // expected hits per tile (0.875 kCap)
 constexpr int kMaxFan = 512;                  // runs per group
-constexpr uint32_t kInterpFan = 192;          // from this fan-in on the partition search interpolates over the whole run first
-
-struct LevelDev {
-    const uint32_t* roff;    // [R+1] run offsets of this level
-    uint32_t* gfirst;        // [G+1] first run of each group
-    uint32_t* tbase;         // [G+1] exclusive prefix of tiles per group
-    uint32_t* sbase;         // [G+1] exclusive prefix of split-table entries per group ((tiles+1) * K)
-    uint64_t* gT0;           // [G] smallest key of the group
-    uint64_t* gDT;           // [G] tile width in key units (>= 1)
-    uint32_t* splits;        // split table
-    uint32_t* roff_next;     // [G+1] run offsets of the next level (= group boundaries)
-    uint4* tile_desc;        // [tiles] {group, first run, runs K, tile k of the group}: one load instead of a chain
-    uint2* tile_desc2;       // [tiles] {split-table offset of the tile's row, tile_base index}
-    uint32_t* tile_base;     // [tiles + G + 1] hits of the group before tile k (nt + 1 entries per group, zeroed, summed by atomics)
-    uint32_t R, G, F;
-};
+constexpr uint32_t kInterpFan = 192;
+constexpr int kFastCap = 4096;                // = kFCap of tt_merge_fast.cuh (checked there)          // from this fan-in on the partition search interpolates over the whole run first
 
 __host__ __device__ inline uint32_t tiles_for(uint32_t n_g) { return (n_g + kTileTarget - 1) / kTileTarget; }
 
@@ -109,6 +97,8 @@ __global__ void __launch_bounds__(1024) merge_setup_kernel(LevelDev lv, const ui
             uint64_t dt = nt ? (kmax >= kmin ? (kmax - kmin) / nt + 1 : 1) : 1;
             if (dt == 0) dt = ~0ull;  // one tile over the whole key range, 2^64 - 1: the + 1 wrapped
             lv.gDT[g] = dt;
+            // the fast tile kernel's bucket map: bucket = hi32((key - Ta) * scale) < kFastCap for key - Ta < dt
+            lv.gScale[g] = (dt > (uint64_t)kFastCap && dt <= 0xFFFFFFFFull) ? (uint32_t)(((uint64_t)kFastCap << 32) / dt) : 0u;
             lv.roff_next[g] = lv.roff[r0];
         }
     }
@@ -641,24 +631,20 @@ __device__ __forceinline__ uint32_t sort_any(MergeSmem& sm, const uint4* __restr
                              prev_pre, status, phase);
 }
 
+// The general tile: any density, any key span, tie blocks (see the file header).  `tile` indexes tile_desc.
 template <bool kPerm>
-__global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, const uint4* __restrict__ in,
-                                                                  uint4* __restrict__ out,
-                                                                  const uint32_t* __restrict__ perm_in,
-                                                                  uint32_t* __restrict__ perm_out, int check_runs,
-                                                                  int32_t* __restrict__ status) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    MergeSmem& sm = *reinterpret_cast<MergeSmem*>(smem_raw);
+__device__ void merge_tile_general(MergeSmem& sm, const LevelDev& lv, uint32_t tile, const uint4* __restrict__ in,
+                                   uint4* __restrict__ out, const uint32_t* __restrict__ perm_in,
+                                   uint32_t* __restrict__ perm_out, int check_runs, int32_t* __restrict__ status,
+                                   uint32_t& phase) {
     const uint32_t tid = threadIdx.x;
-    if (tid == 0) mbar_init(&sm.mbar, 1);
-    uint32_t phase = 0;
     {   // the bucket array is cleared while the tile's description is on its way; the barrier below orders it
         uint4* z = reinterpret_cast<uint4*>(sm.cs);
 #pragma unroll
         for (int i = 0; i < kCap / 4 / kMThreads; ++i) z[tid + i * kMThreads] = make_uint4(0, 0, 0, 0);
     }
-    const uint4 td = lv.tile_desc[blockIdx.x];
-    const uint2 td2 = lv.tile_desc2[blockIdx.x];
+    const uint4 td = lv.tile_desc[tile];
+    const uint2 td2 = lv.tile_desc2[tile];
     const uint32_t g = td.x, r0 = td.y, K = td.z, k = td.w;
     const uint32_t* row0 = lv.splits + td2.x;
     const uint32_t* row1 = row0 + K;
@@ -775,12 +761,42 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_tile_kernel(LevelDev lv, c
     }
 }
 
+// The tiles the fast kernel (tt_merge_fast.cuh) left over: a fixed grid walks the list.
+template <bool kPerm>
+__global__ void __launch_bounds__(kMThreads, 2) merge_slow_kernel(LevelDev lv, const uint4* __restrict__ in,
+                                                                  uint4* __restrict__ out,
+                                                                  const uint32_t* __restrict__ perm_in,
+                                                                  uint32_t* __restrict__ perm_out, int check_runs,
+                                                                  int32_t* __restrict__ status) {
+    const uint32_t n_slow = *lv.slow_cnt;
+    if (blockIdx.x >= n_slow) return;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    MergeSmem& sm = *reinterpret_cast<MergeSmem*>(smem_raw);
+    if (threadIdx.x == 0) mbar_init(&sm.mbar, 1);
+    uint32_t phase = 0;
+    for (uint32_t i = blockIdx.x; i < n_slow; i += gridDim.x) {
+        merge_tile_general<kPerm>(sm, lv, lv.slow_list[i], in, out, perm_in, perm_out, check_runs, status, phase);
+        __syncthreads();
+    }
+}
+
+#include "tt_merge_fast.cuh"
+static_assert(kFCap == kFastCap, "plan and fast kernel agree on the bucket count");
+
 // ---- host side: plan mirror -----------------------------------------------------------------------------
+// Only counts: the host never needs the per-level offset arrays after sizing, so the plan of the last call is kept
+// per host thread and reused while the offsets are unchanged (a hot call then allocates nothing).
 struct LevelHost {
-    std::vector<uint32_t> roff;  // run offsets of this level
     uint32_t R, G, F, tiles, split_entries;
     uint32_t kmax;               // most runs in one group of this level
-    std::vector<uint32_t> next;  // group boundaries
+};
+
+struct PlanCache {
+    std::vector<uint32_t> seg, runs;  // the offsets the plan was made for
+    uint32_t n = 0;
+    bool valid = false;
+    std::vector<LevelHost> levels;
+    std::vector<uint32_t> roff, next;  // scratch of build_plan
 };
 
 static uint32_t lower_bound_u32(const std::vector<uint32_t>& v, uint32_t R, uint32_t x) {
@@ -789,32 +805,14 @@ static uint32_t lower_bound_u32(const std::vector<uint32_t>& v, uint32_t R, uint
     return lo;
 }
 
-static void plan_level(LevelHost& L, const uint32_t* h_seg, uint32_t n_seg, uint32_t n) {
-    L.tiles = 0; L.split_entries = 0; L.G = 0;
-    L.next.clear();
-    for (uint32_t s = 0; s < n_seg; ++s) {
-        const uint32_t r0 = lower_bound_u32(L.roff, L.R, h_seg[s]);
-        const uint32_t r1 = s + 1 == n_seg ? L.R : lower_bound_u32(L.roff, L.R, h_seg[s + 1]);
-        for (uint32_t r = r0; r < r1; r += L.F) {
-            const uint32_t re = r + L.F < r1 ? r + L.F : r1;
-            const uint32_t nt = tiles_for(L.roff[re] - L.roff[r]);
-            L.tiles += nt;
-            L.split_entries += nt ? (nt + 1) * (re - r) : 0;
-            L.next.push_back(L.roff[r]);
-            ++L.G;
-        }
-    }
-    L.next.push_back(n);
-}
-
-static void build_plan(std::vector<LevelHost>& levels, uint32_t n, const uint32_t* h_seg, uint32_t n_seg,
-                       const uint32_t* h_runs, uint32_t n_runs) {
+static void build_plan(PlanCache& pc, uint32_t n, const uint32_t* h_seg, uint32_t n_seg, const uint32_t* h_runs,
+                       uint32_t n_runs) {
     // largest number of runs in one segment decides the number of levels and the fan-in
-    std::vector<uint32_t> roff(h_runs, h_runs + n_runs + 1);
+    pc.roff.assign(h_runs, h_runs + n_runs + 1);
     uint32_t pmax = 1;
     for (uint32_t s = 0; s < n_seg; ++s) {
-        const uint32_t r0 = lower_bound_u32(roff, n_runs, h_seg[s]);
-        const uint32_t r1 = s + 1 == n_seg ? n_runs : lower_bound_u32(roff, n_runs, h_seg[s + 1]);
+        const uint32_t r0 = lower_bound_u32(pc.roff, n_runs, h_seg[s]);
+        const uint32_t r1 = s + 1 == n_seg ? n_runs : lower_bound_u32(pc.roff, n_runs, h_seg[s + 1]);
         if (r1 - r0 > pmax) pmax = r1 - r0;
     }
     uint32_t nlev = 1;
@@ -829,29 +827,59 @@ static void build_plan(std::vector<LevelHost>& levels, uint32_t n, const uint32_
             ++F;
         }
     }
-    levels.clear();
-    LevelHost L;
-    L.roff = roff; L.R = n_runs; L.F = F;
+    pc.levels.clear();
+    uint32_t R = n_runs;
     uint32_t pm = pmax;  // most runs of one segment at this level
     for (uint32_t l = 0; l < nlev; ++l) {
-        plan_level(L, h_seg, n_seg, n);
+        LevelHost L;
+        L.R = R; L.F = F; L.tiles = 0; L.split_entries = 0; L.G = 0;
+        pc.next.clear();
+        for (uint32_t s = 0; s < n_seg; ++s) {
+            const uint32_t r0 = lower_bound_u32(pc.roff, R, h_seg[s]);
+            const uint32_t r1 = s + 1 == n_seg ? R : lower_bound_u32(pc.roff, R, h_seg[s + 1]);
+            for (uint32_t r = r0; r < r1; r += F) {
+                const uint32_t re = r + F < r1 ? r + F : r1;
+                const uint32_t nt = tiles_for(pc.roff[re] - pc.roff[r]);
+                L.tiles += nt;
+                L.split_entries += nt ? (nt + 1) * (re - r) : 0;
+                pc.next.push_back(pc.roff[r]);
+                ++L.G;
+            }
+        }
+        pc.next.push_back(n);
         L.kmax = pm < F ? pm : F;
         pm = (pm + F - 1) / F;
-        levels.push_back(L);
-        LevelHost N;
-        N.roff = L.next; N.R = L.G; N.F = F;
-        L = N;
+        pc.levels.push_back(L);
+        pc.roff.swap(pc.next);
+        R = L.G;
     }
 }
 
+static const std::vector<LevelHost>& plan_for(uint32_t n, const uint32_t* h_seg, uint32_t n_seg, const uint32_t* h_runs,
+                                              uint32_t n_runs) {
+    thread_local PlanCache pc;
+    if (pc.valid && pc.n == n && pc.seg.size() == (size_t)n_seg + 1 && pc.runs.size() == (size_t)n_runs + 1 &&
+        std::memcmp(pc.seg.data(), h_seg, ((size_t)n_seg + 1) * 4) == 0 &&
+        std::memcmp(pc.runs.data(), h_runs, ((size_t)n_runs + 1) * 4) == 0)
+        return pc.levels;
+    pc.valid = false;
+    pc.seg.assign(h_seg, h_seg + n_seg + 1);
+    pc.runs.assign(h_runs, h_runs + n_runs + 1);
+    pc.n = n;
+    build_plan(pc, n, h_seg, n_seg, h_runs, n_runs);
+    pc.valid = true;
+    return pc.levels;
+}
+
+constexpr int kMaxLevels = 4;  // 512^4 runs
+
 struct MergeWs {
-    std::vector<LevelDev> dev;
+    LevelDev dev[kMaxLevels];
     uint4* tmp[2];
     uint32_t* ptmp[2];
 };
 
 static void carve(Arena& a, const std::vector<LevelHost>& levels, uint32_t n, bool perm, MergeWs& w) {
-    w.dev.resize(levels.size());
     for (size_t l = 0; l < levels.size(); ++l) {
         const LevelHost& L = levels[l];
         LevelDev& d = w.dev[l];
@@ -861,11 +889,15 @@ static void carve(Arena& a, const std::vector<LevelHost>& levels, uint32_t n, bo
         d.sbase = a.take<uint32_t>(L.G + 1);
         d.gT0 = a.take<uint64_t>(L.G + 1);
         d.gDT = a.take<uint64_t>(L.G + 1);
+        d.gScale = a.take<uint32_t>(L.G + 1);
         d.splits = a.take<uint32_t>((size_t)L.split_entries + 1);
         d.roff_next = a.take<uint32_t>(L.G + 1);
         d.tile_desc = a.take<uint4>((size_t)L.tiles + 1);
         d.tile_desc2 = a.take<uint2>((size_t)L.tiles + 1);
-        d.tile_base = a.take<uint32_t>((size_t)L.tiles + L.G + 1);
+        d.tile_base = a.take<uint32_t>((size_t)L.tiles + L.G + 2);  // + the slow-tile counter: one memset clears both
+        d.slow_cnt = d.tile_base ? d.tile_base + ((size_t)L.tiles + L.G + 1) : nullptr;
+        d.slow_list = a.take<uint32_t>((size_t)L.tiles + 1);
+        d.tile_open = a.take<uint8_t>((size_t)L.tiles + 1);
     }
     const size_t nlev = levels.size();
     w.tmp[0] = nlev > 1 ? a.take<uint4>(n) : nullptr;
@@ -875,43 +907,53 @@ static void carve(Arena& a, const std::vector<LevelHost>& levels, uint32_t n, bo
 }
 
 size_t merge_ws_bytes(uint32_t n, const uint32_t* h_seg, uint32_t n_seg, const uint32_t* h_runs, uint32_t n_runs) {
-    std::vector<LevelHost> levels;
-    build_plan(levels, n, h_seg, n_seg, h_runs, n_runs);
+    const std::vector<LevelHost>& levels = plan_for(n, h_seg, n_seg, h_runs, n_runs);
+    if (levels.size() > (size_t)kMaxLevels) return ~size_t(0);
     Arena a(nullptr);
     MergeWs w;
     carve(a, levels, n, true, w);
     return a.off;
 }
 
+static int merge_attrs() {
+    TT_CUDA_OK(cudaFuncSetAttribute(merge_slow_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MergeSmem)));
+    TT_CUDA_OK(cudaFuncSetAttribute(merge_slow_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MergeSmem)));
+    TT_CUDA_OK(cudaFuncSetAttribute(merge_fast_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
+    TT_CUDA_OK(cudaFuncSetAttribute(merge_fast_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
+    TT_CUDA_OK(cudaFuncSetAttribute(merge_fast_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
+    TT_CUDA_OK(cudaFuncSetAttribute(merge_fast_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(FastSmem)));
+    return TT_OK;
+}
+
 int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, const uint32_t* d_seg_offsets,
                     const uint32_t* h_seg, uint32_t n_seg, const uint32_t* d_run_offsets, const uint32_t* h_runs,
-                    uint32_t n_runs, void* d_ws, int32_t* d_status, cudaStream_t s) {
-    std::vector<LevelHost> levels;
-    build_plan(levels, n, h_seg, n_seg, h_runs, n_runs);
+                    uint32_t n_runs, void* d_ws, int32_t* d_status, cudaStream_t s, const FuseL1* fuse, MergeLast* last) {
+    const std::vector<LevelHost>& levels = plan_for(n, h_seg, n_seg, h_runs, n_runs);
+    const size_t nlev = levels.size();
+    if (nlev > (size_t)kMaxLevels) return TT_E_INVAL;
     Arena a(d_ws);
     MergeWs w;
     carve(a, levels, n, true, w);
-    static bool attr_done = false;
-    if (!attr_done) {
-        TT_CUDA_OK(cudaFuncSetAttribute(merge_tile_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MergeSmem)));
-        TT_CUDA_OK(cudaFuncSetAttribute(merge_tile_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(MergeSmem)));
-        attr_done = true;
-    }
-    const size_t nlev = levels.size();
+    int rc = once_per_device(kSlotMerge, merge_attrs);
+    if (rc != TT_OK) return rc;
+    const uint32_t slow_grid = 2u * (uint32_t)sm_count();
     const uint4* src = (const uint4*)d_in;
     const uint32_t* psrc = nullptr;
+    FuseL1 none;
+    none.flags = nullptr; none.lc = 0; none.q_thresh = 0;
     for (size_t l = 0; l < nlev; ++l) {
         LevelDev& d = w.dev[l];
         d.roff = l == 0 ? d_run_offsets : w.dev[l - 1].roff_next;
-        const bool last = l + 1 == nlev;
-        uint4* dst = last ? (uint4*)d_out : w.tmp[l & 1];
-        uint32_t* pdst = d_perm ? (last ? d_perm : w.ptmp[l & 1]) : nullptr;
+        const bool is_last = l + 1 == nlev;
+        const bool fused = is_last && fuse && fuse->flags;
+        uint4* dst = is_last ? (uint4*)d_out : w.tmp[l & 1];
+        uint32_t* pdst = d_perm ? (is_last ? d_perm : w.ptmp[l & 1]) : nullptr;
         prof_mark(s, l == 0 ? "sort.merge_plan0" : "sort.merge_plan1");
         TT_K(merge_groups_kernel)<<<1, 1024, 0, s>>>(d, d_seg_offsets, n_seg);
         TT_K(merge_setup_kernel)<<<1, 1024, 0, s>>>(d, src, n);
+        TT_CUDA_OK(cudaMemsetAsync(d.tile_base, 0, ((size_t)levels[l].tiles + levels[l].G + 2) * sizeof(uint32_t), s));
         if (levels[l].split_entries) {
             prof_mark(s, l == 0 ? "sort.merge_partition0" : "sort.merge_partition1");
-            TT_CUDA_OK(cudaMemsetAsync(d.tile_base, 0, ((size_t)levels[l].tiles + levels[l].G + 1) * sizeof(uint32_t), s));
             if (levels[l].kmax >= kInterpFan)
                 TT_K(merge_partition_kernel<true>)<<<div_up(levels[l].split_entries, 256), 256, 0, s>>>(d, src, levels[l].split_entries);
             else
@@ -919,11 +961,19 @@ int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_
         }
         if (levels[l].tiles) {
             prof_mark(s, l == 0 ? "sort.merge_tile0" : "sort.merge_tile1");
-            if (d_perm)
-                TT_K(merge_tile_kernel<true>)<<<levels[l].tiles, kMThreads, sizeof(MergeSmem), s>>>(d, src, dst, psrc, pdst, l == 0, d_status);
-            else
-                TT_K(merge_tile_kernel<false>)<<<levels[l].tiles, kMThreads, sizeof(MergeSmem), s>>>(d, src, dst, nullptr, nullptr, l == 0, d_status);
+            const uint32_t nt = levels[l].tiles;
+            const int chk = l == 0;
+            if (d_perm) {
+                if (fused) TT_K((merge_fast_kernel<true, true>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, src, dst, psrc, pdst, chk, *fuse, d_status);
+                else TT_K((merge_fast_kernel<true, false>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, src, dst, psrc, pdst, chk, none, d_status);
+                TT_K(merge_slow_kernel<true>)<<<slow_grid, kMThreads, sizeof(MergeSmem), s>>>(d, src, dst, psrc, pdst, chk, d_status);
+            } else {
+                if (fused) TT_K((merge_fast_kernel<false, true>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, src, dst, nullptr, nullptr, chk, *fuse, d_status);
+                else TT_K((merge_fast_kernel<false, false>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, src, dst, nullptr, nullptr, chk, none, d_status);
+                TT_K(merge_slow_kernel<false>)<<<slow_grid, kMThreads, sizeof(MergeSmem), s>>>(d, src, dst, nullptr, nullptr, chk, d_status);
+            }
         }
+        if (is_last && last) { last->lv = d; last->tiles = levels[l].tiles; }
         src = dst;
         psrc = pdst;
     }

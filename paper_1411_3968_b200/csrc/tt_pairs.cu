@@ -304,6 +304,12 @@ __global__ void __launch_bounds__(kCThreads) l0_combine_kernel(const uint8_t* __
 
 }  // namespace tt
 
+static int pairs_attrs() {
+    TT_CUDA_OK(cudaFuncSetAttribute(tt::pair_seeds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(sizeof(tt::PairSmem) + tt::kPAdjSmem * tt::kPAdjSmem)));
+    return TT_OK;
+}
+
 extern "C" int tt_pair_seeds(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
                              const uint8_t* d_adj, uint32_t pmts_per_tower, int64_t sc_window_ps, int64_t fc_window_ps,
                              int64_t afc_window_ps, uint8_t* d_bits, void* stream) {
@@ -320,11 +326,9 @@ extern "C" int tt_pair_seeds(const tt_hit* d_sorted, uint32_t n, const uint32_t*
     w.wmax = w.afc > w.wmax ? w.afc : w.wmax;
     w.rcp = ((1ull << 32) + pmts_per_tower - 1) / pmts_per_tower;
     const size_t smem = sizeof(PairSmem) + (pmts_per_tower <= kPAdjSmem ? (size_t)pmts_per_tower * pmts_per_tower : 0);
-    static bool attr_done = false;
-    if (!attr_done) {
-        TT_CUDA_OK(cudaFuncSetAttribute(pair_seeds_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        (int)(sizeof(PairSmem) + kPAdjSmem * kPAdjSmem)));
-        attr_done = true;
+    {
+        const int rc = once_per_device(kSlotPairs, pairs_attrs);
+        if (rc != TT_OK) return rc;
     }
     prof_mark(s, "pairs.seeds");
     TT_K(pair_seeds_kernel)<<<div_up(n, kPTile), kPThreads, smem, s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,

@@ -6,7 +6,7 @@
 //   L2   PAPER.md:27-29 ("time-space correlation between PMT hits within a time interval less than
 //        3 us"); north_star: ">= N L1 hits pairwise satisfying |dt| <= dt_max(pmt_i, pmt_j)"
 //   seeds PAPER.md:67, 81 ("sends all trigger seeds")
-#include "tt_common.cuh"
+#include "tt_merge.cuh"
 
 namespace tt {
 
@@ -225,6 +225,92 @@ __global__ void __launch_bounds__(kL1Threads) l1_tile_kernel(const uint4* __rest
     if (lane == 0) s_red[tid >> 5] = cnt;
     __syncthreads();
     if (tid == 0) {
+        uint32_t c = 0;
+#pragma unroll
+        for (int w = 0; w < kL1Threads / 32; ++w) c += s_red[w];
+        tile_cnt[blockIdx.x] = c;
+    }
+}
+
+// ---- fused path (tt_sort_trigger_slice): the last merge level wrote Q / LC / L1 for every hit from what its own
+// time tile holds (merge_fast_kernel<.., true>).  A partner in a neighbouring tile was not visible there, so the
+// hits within LC of the last hit before their tile or of the first hit after it -- and every hit of a tile the general
+// merge kernel sorted (tile_open) -- get their flag byte from an exact scan of the sorted array here.  One warp per
+// tile.  At the last level a group is a whole segment, so [gs, ge) bounds the scans.
+constexpr int kBndWarps = 8;
+
+__device__ __forceinline__ void l1_exact(const uint4* __restrict__ hits, uint32_t i, uint32_t gs, uint32_t ge, uint64_t lc,
+                                         uint32_t q_thresh, uint8_t* __restrict__ flags) {
+    const uint4 v = __ldg(hits + i);
+    uint32_t f = (v.w & 0xFFFFu) >= q_thresh ? (uint32_t)TT_Q : 0u;
+    if (lc_scan_global(hits, hit_time(v), v.z, i, i + 1, gs, ge, lc)) f |= TT_LC;
+    if (f) f |= TT_L1;
+    flags[i] = (uint8_t)f;
+}
+
+__global__ void __launch_bounds__(kBndWarps * 32) l1_boundary_kernel(LevelDev lv, uint32_t n_tiles,
+                                                                     const uint4* __restrict__ hits, uint64_t lc,
+                                                                     uint32_t q_thresh, uint8_t* __restrict__ flags) {
+    const uint32_t lane = threadIdx.x & 31u;
+    const uint32_t tile = blockIdx.x * kBndWarps + (threadIdx.x >> 5);
+    if (tile >= n_tiles) return;
+    const uint4 td = lv.tile_desc[tile];
+    const uint2 td2 = lv.tile_desc2[tile];
+    const uint32_t gs = lv.roff[td.y], ge = lv.roff[td.y + td.z];
+    const uint32_t tb0 = lv.tile_base[td2.y], tb1 = lv.tile_base[td2.y + 1];
+    uint32_t b0 = gs + tb0, b1 = gs + tb1;  // the tile's range of the sorted array
+    if (b0 > ge) b0 = ge;                    // only with unsorted runs (output unspecified, accesses stay in range)
+    if (b1 > ge) b1 = ge;
+    if (b1 <= b0) return;
+    if (lv.tile_open[tile]) {
+        for (uint32_t i = b0 + lane; i < b1; i += 32) l1_exact(hits, i, gs, ge, lc, q_thresh, flags);
+        return;
+    }
+    const bool has_prev = b0 > gs, has_next = b1 < ge;
+    const int64_t t_prev = has_prev ? hit_time(__ldg(hits + b0 - 1)) : 0;
+    const int64_t t_next = has_next ? hit_time(__ldg(hits + b1)) : 0;
+    if (has_prev) {  // head: hits within LC of the last hit before the tile
+        for (uint32_t base = b0; base < b1; base += 32) {
+            const uint32_t i = base + lane;
+            const bool open = i < b1 && udiff(hit_time(__ldg(hits + i)), t_prev) <= lc;
+            if (open) l1_exact(hits, i, gs, ge, lc, q_thresh, flags);
+            if (!__all_sync(0xffffffffu, open)) break;
+        }
+    }
+    if (has_next) {  // tail: hits within LC of the first hit after the tile (not those the head loop already did)
+        for (uint32_t base = b1; base > b0;) {
+            const bool valid = base - b0 > lane;
+            const uint32_t i = base - 1u - lane;
+            bool open = false;
+            if (valid) {
+                const int64_t t = hit_time(__ldg(hits + i));
+                open = udiff(t_next, t) <= lc;
+                if (open && !(has_prev && udiff(t, t_prev) <= lc)) l1_exact(hits, i, gs, ge, lc, q_thresh, flags);
+            }
+            if (!__all_sync(0xffffffffu, open)) break;
+            base -= 32;
+        }
+    }
+}
+
+// L1 hits per block of kL1Tile flag bytes (the fused path has no l1_tile_kernel to count them)
+__global__ void __launch_bounds__(kL1Threads) l1_count_kernel(const uint8_t* __restrict__ flags, uint32_t n,
+                                                              uint32_t* __restrict__ tile_cnt) {
+    __shared__ uint32_t s_red[kL1Threads / 32];
+    const uint32_t i0 = blockIdx.x * (uint32_t)kL1Tile + threadIdx.x * kL1Per;
+    uint32_t cnt = 0;
+    if (i0 < n) {
+        if (i0 + kL1Per <= n && (((uintptr_t)(flags + i0)) & 15) == 0) {
+            const uint4 v = *reinterpret_cast<const uint4*>(flags + i0);
+            cnt = __popc(v.x & 0x04040404u) + __popc(v.y & 0x04040404u) + __popc(v.z & 0x04040404u) + __popc(v.w & 0x04040404u);
+        } else {
+            for (uint32_t k = 0; k < (uint32_t)kL1Per && i0 + k < n; ++k) cnt += (flags[i0 + k] & TT_L1) ? 1u : 0u;
+        }
+    }
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    if ((threadIdx.x & 31) == 0) s_red[threadIdx.x >> 5] = cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) {
         uint32_t c = 0;
 #pragma unroll
         for (int w = 0; w < kL1Threads / 32; ++w) c += s_red[w];
@@ -940,11 +1026,18 @@ static void trigger_plan(Arena& a, uint32_t n, TriggerPlan& p) {
 
 using namespace tt;
 
-extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets,
-                                const uint32_t* h_seg_offsets, uint32_t n_seg, const tt_geometry* g,
-                                const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds, uint32_t seed_cap,
-                                uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes, int32_t* d_status, void* stream) {
-    if (!ws_bytes || !p || !g || n_seg < 1 || !h_seg_offsets) return TT_E_INVAL;
+static int trigger_attrs() {
+    TT_CUDA_OK(cudaFuncSetAttribute(l2_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(sizeof(WideSmem) * kL2Warps)));
+    TT_CUDA_OK(cudaFuncSetAttribute(l1_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(L1Smem)));
+    TT_CUDA_OK(cudaFuncSetAttribute(l2_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    (int)(sizeof(RowSmem) + kPairBytesMax)));
+    return TT_OK;
+}
+
+static int trigger_args_ok(uint32_t n, const uint32_t* h_seg_offsets, uint32_t n_seg, const tt_geometry* g,
+                           const tt_params* p) {
+    if (!p || !g || n_seg < 1 || !h_seg_offsets) return TT_E_INVAL;
     if (p->l2_multiplicity < 1 || p->l2_multiplicity > TT_MAX_MULTIPLICITY || p->l2_mode > 1 || p->reserved != 0 ||
         p->lc_window_ps < 0 || p->l2_window_ps < 0 || p->event_half_ps < 0)
         return TT_E_INVAL;
@@ -952,6 +1045,71 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     if (h_seg_offsets[0] != 0 || h_seg_offsets[n_seg] != n) return TT_E_INVAL;
     for (uint32_t s = 0; s < n_seg; ++s)
         if (h_seg_offsets[s] > h_seg_offsets[s + 1]) return TT_E_INVAL;
+    return TT_OK;
+}
+
+// Everything of tt_trigger_slice.  last == nullptr: L1 by l1_tile_kernel.  last != nullptr: the last merge level has
+// written the in-tile L1 flags (fused call); the tile edges are finished here.
+static int trigger_run(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
+                       const tt_geometry* g, const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds, uint32_t seed_cap,
+                       uint32_t* d_n_seeds, void* d_ws, int32_t* d_status, cudaStream_t s, const MergeLast* last) {
+    Arena a(d_ws);
+    TriggerPlan plan;
+    trigger_plan(a, n, plan);
+    int rc = once_per_device(kSlotTrigger, trigger_attrs);
+    if (rc != TT_OK) return rc;
+    const uint32_t sms = (uint32_t)sm_count();
+    if (!last) {
+        prof_mark(s, "trig.l1_flags");
+        TT_K(l1_tile_kernel)<<<plan.nblk, kL1Threads, sizeof(L1Smem), s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,
+                                                        (uint64_t)p->lc_window_ps, p->q_thresh, d_flags, plan.blk_cnt);
+    } else {
+        prof_mark(s, "trig.l1_edges");
+        if (last->tiles)
+            TT_K(l1_boundary_kernel)<<<div_up(last->tiles, kBndWarps), kBndWarps * 32, 0, s>>>(
+                last->lv, last->tiles, (const uint4*)d_sorted, (uint64_t)p->lc_window_ps, p->q_thresh, d_flags);
+        TT_K(l1_count_kernel)<<<plan.nblk, kL1Threads, 0, s>>>(d_flags, n, plan.blk_cnt);
+    }
+    prof_mark(s, "trig.l1_scan");
+    rc = exclusive_scan_u32(plan.blk_cnt, plan.blk_cnt, plan.nblk, plan.scan_scratch, plan.m_total, s);
+    if (rc != TT_OK) return rc;
+    prof_mark(s, "trig.l1_compact");
+    TT_K(l1_compact_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1,
+                                                         g->dev.n_pmt, g->dev.ppt, d_status);
+    prof_mark(s, "trig.l2_rows");
+    TT_CUDA_OK(cudaMemsetAsync(plan.slow_cnt, 0, 4 * sizeof(uint32_t), s));
+    const uint32_t nt2 = g->dev.n_tower * g->dev.n_tower;
+    const uint32_t pair_smem = (g->dev.n_tower > 1 && nt2 <= (uint32_t)kPairBytesMax && g->dev.n_blocks <= 255u) ? 1u : 0u;
+    const size_t rows_smem = sizeof(RowSmem) + (pair_smem ? ((nt2 + 15u) & ~15u) : 0);
+    TT_K(l2_rows_kernel)<<<sms * 4, kRowTile, rows_smem, s>>>(
+        plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps, p->l2_multiplicity, p->l2_mode,
+        pair_smem, d_flags, plan.l2bit, plan.rows, plan.slow_list, plan.slow_cnt);
+    prof_mark(s, "trig.l2_clique");
+    TT_K(l2_clique_kernel)<<<sms * 6, kClqTile, 0, s>>>(plan.l1, plan.m_total, plan.rows, p->l2_multiplicity, p->l2_mode,
+                                                        d_flags, plan.l2bit, plan.slow_list, plan.slow_cnt);
+    prof_mark(s, "trig.l2_wide");
+    TT_K(l2_wide_kernel)<<<sms * 4, kL2Warps * 32, sizeof(WideSmem) * kL2Warps, s>>>(
+        plan.l1, plan.m_total, plan.slow_list, plan.slow_cnt, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps,
+        p->l2_multiplicity, p->l2_mode, d_flags, plan.l2bit, d_status);
+    prof_counter(s, "l1_hits", plan.m_total);
+    prof_counter(s, "l2_slow_items", plan.slow_cnt);
+    prof_mark(s, "trig.seeds");
+    TT_K(seed_count_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.m_total, plan.seed_cnt);
+    TT_K(count_scan_kernel)<<<1, 1024, 0, s>>>(plan.seed_cnt, kSeedBlocks, d_n_seeds, seed_cap, TT_S_SEED_OVERFLOW, d_status);
+    TT_K(seed_write_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.l1, plan.m_total, plan.seed_cnt, d_seeds,
+                                                           seed_cap, d_flags);
+    prof_end(s);
+    TT_LAUNCH_OK();
+    return TT_OK;
+}
+
+extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets,
+                                const uint32_t* h_seg_offsets, uint32_t n_seg, const tt_geometry* g,
+                                const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds, uint32_t seed_cap,
+                                uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes, int32_t* d_status, void* stream) {
+    if (!ws_bytes) return TT_E_INVAL;
+    int rc = trigger_args_ok(n, h_seg_offsets, n_seg, g, p);
+    if (rc != TT_OK) return rc;
     Arena sizing(nullptr);
     TriggerPlan plan;
     trigger_plan(sizing, n, plan);
@@ -968,49 +1126,63 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
         TT_CUDA_OK(cudaMemsetAsync(d_n_seeds, 0, sizeof(uint32_t), s));
         return TT_OK;
     }
-    Arena a(d_ws);
-    trigger_plan(a, n, plan);
-    static bool attr_done = false;
-    if (!attr_done) {
-        TT_CUDA_OK(cudaFuncSetAttribute(l2_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        (int)(sizeof(WideSmem) * kL2Warps)));
-        TT_CUDA_OK(cudaFuncSetAttribute(l1_tile_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(L1Smem)));
-        TT_CUDA_OK(cudaFuncSetAttribute(l2_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        (int)(sizeof(RowSmem) + kPairBytesMax)));
-        attr_done = true;
-    }
-    prof_mark(s, "trig.l1_flags");
-    TT_K(l1_tile_kernel)<<<plan.nblk, kL1Threads, sizeof(L1Smem), s>>>((const uint4*)d_sorted, n, d_seg_offsets, n_seg,
-                                                    (uint64_t)p->lc_window_ps, p->q_thresh, d_flags, plan.blk_cnt);
-    prof_mark(s, "trig.l1_scan");
-    int rc = exclusive_scan_u32(plan.blk_cnt, plan.blk_cnt, plan.nblk, plan.scan_scratch, plan.m_total, s);
+    return trigger_run(d_sorted, n, d_seg_offsets, n_seg, g, p, d_flags, d_seeds, seed_cap, d_n_seeds, d_ws, d_status, s,
+                       nullptr);
+}
+
+// tt_sort_slice + tt_trigger_slice in one call (last bullet): same outputs, byte for byte.  With runs
+// given, L1 is evaluated by the last merge level on its sorted tile in shared memory, so the sorted array is not read
+// again for it; without runs (radix sort) the two calls simply run back to back.
+extern "C" int tt_sort_trigger_slice(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n,
+                                     const uint32_t* d_seg_offsets, const uint32_t* h_seg_offsets, uint32_t n_seg,
+                                     const uint32_t* d_run_offsets, const uint32_t* h_run_offsets, uint32_t n_runs,
+                                     const tt_geometry* g, const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds,
+                                     uint32_t seed_cap, uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes,
+                                     int32_t* d_status, void* stream) {
+    if (!ws_bytes) return TT_E_INVAL;
+    int rc = trigger_args_ok(n, h_seg_offsets, n_seg, g, p);
     if (rc != TT_OK) return rc;
-    prof_mark(s, "trig.l1_compact");
-    TT_K(l1_compact_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1,
-                                                         g->dev.n_pmt, g->dev.ppt, d_status);
-    prof_mark(s, "trig.l2_rows");
-    TT_CUDA_OK(cudaMemsetAsync(plan.slow_cnt, 0, 4 * sizeof(uint32_t), s));
-    const uint32_t nt2 = g->dev.n_tower * g->dev.n_tower;
-    const uint32_t pair_smem = (g->dev.n_tower > 1 && nt2 <= (uint32_t)kPairBytesMax && g->dev.n_blocks <= 255u) ? 1u : 0u;
-    const size_t rows_smem = sizeof(RowSmem) + (pair_smem ? ((nt2 + 15u) & ~15u) : 0);
-    TT_K(l2_rows_kernel)<<<kSMs * 4, kRowTile, rows_smem, s>>>(
-        plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps, p->l2_multiplicity, p->l2_mode,
-        pair_smem, d_flags, plan.l2bit, plan.rows, plan.slow_list, plan.slow_cnt);
-    prof_mark(s, "trig.l2_clique");
-    TT_K(l2_clique_kernel)<<<kSMs * 6, kClqTile, 0, s>>>(plan.l1, plan.m_total, plan.rows, p->l2_multiplicity, p->l2_mode,
-                                                        d_flags, plan.l2bit, plan.slow_list, plan.slow_cnt);
-    prof_mark(s, "trig.l2_wide");
-    TT_K(l2_wide_kernel)<<<kSMs * 4, kL2Warps * 32, sizeof(WideSmem) * kL2Warps, s>>>(
-        plan.l1, plan.m_total, plan.slow_list, plan.slow_cnt, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps,
-        p->l2_multiplicity, p->l2_mode, d_flags, plan.l2bit, d_status);
-    prof_counter(s, "l1_hits", plan.m_total);
-    prof_counter(s, "l2_slow_items", plan.slow_cnt);
-    prof_mark(s, "trig.seeds");
-    TT_K(seed_count_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.m_total, plan.seed_cnt);
-    TT_K(count_scan_kernel)<<<1, 1024, 0, s>>>(plan.seed_cnt, kSeedBlocks, d_n_seeds, seed_cap, TT_S_SEED_OVERFLOW, d_status);
-    TT_K(seed_write_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(plan.l2bit, plan.l1, plan.m_total, plan.seed_cnt, d_seeds,
-                                                           seed_cap, d_flags);
-    prof_end(s);
-    TT_LAUNCH_OK();
-    return TT_OK;
+    size_t ws_sort = 0, ws_trig = 0;
+    rc = tt_sort_slice(nullptr, nullptr, nullptr, n, nullptr, h_seg_offsets, n_seg, d_run_offsets, h_run_offsets, n_runs,
+                       nullptr, &ws_sort, nullptr, nullptr);
+    if (rc != TT_OK) return rc;
+    rc = tt_trigger_slice(nullptr, n, nullptr, h_seg_offsets, n_seg, g, p, nullptr, nullptr, seed_cap, nullptr, nullptr,
+                          &ws_trig, nullptr, nullptr);
+    if (rc != TT_OK) return rc;
+    ws_sort = (ws_sort + 255) & ~size_t(255);
+    if (!d_ws) {
+        *ws_bytes = ws_sort + ws_trig;
+        return TT_OK;
+    }
+    if (*ws_bytes < ws_sort + ws_trig) return TT_E_WORKSPACE;
+    if (!d_flags || !d_n_seeds || !d_status || (!d_seeds && seed_cap)) return TT_E_INVAL;
+    if (n && (!d_in || !d_out || !d_seg_offsets || d_in == d_out)) return TT_E_INVAL;
+    if (((uintptr_t)d_ws & 255) || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return TT_E_INVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n == 0) {
+        TT_CUDA_OK(cudaMemsetAsync(d_n_seeds, 0, sizeof(uint32_t), s));
+        return TT_OK;
+    }
+    void* d_ws_trig = (char*)d_ws + ws_sort;
+    const bool runs = d_run_offsets != nullptr || h_run_offsets != nullptr;
+    if (!runs) {
+        size_t w = ws_sort;
+        rc = tt_sort_slice(d_in, d_out, d_perm, n, d_seg_offsets, h_seg_offsets, n_seg, nullptr, nullptr, 0, d_ws, &w,
+                           d_status, stream);
+        if (rc != TT_OK) return rc;
+        return trigger_run(d_out, n, d_seg_offsets, n_seg, g, p, d_flags, d_seeds, seed_cap, d_n_seeds, d_ws_trig, d_status,
+                           s, nullptr);
+    }
+    if (!d_run_offsets || !h_run_offsets || n_runs < 1) return TT_E_INVAL;
+    FuseL1 fz;
+    fz.flags = d_flags;
+    fz.lc = (uint64_t)p->lc_window_ps;
+    fz.q_thresh = p->q_thresh;
+    MergeLast last;
+    last.tiles = 0;
+    rc = merge_sort_runs(d_in, d_out, d_perm, n, d_seg_offsets, h_seg_offsets, n_seg, d_run_offsets, h_run_offsets, n_runs,
+                         d_ws, d_status, s, &fz, &last);
+    if (rc != TT_OK) return rc;
+    return trigger_run(d_out, n, d_seg_offsets, n_seg, g, p, d_flags, d_seeds, seed_cap, d_n_seeds, d_ws_trig, d_status, s,
+                       &last);
 }
