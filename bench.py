@@ -227,8 +227,11 @@ def run_ours(args):
 
     def step():
         d_cnt.zero_()
-        ws["s"] = B.tt_sort_slice(d_in, d_out, None, seg, runs, d_st, ws.get("s"))
-        ws["t"] = B.tt_trigger_slice(d_out, seg, geo, prm, d_flags, d_seeds, d_ns, d_st, ws.get("t"))
+        if args.fused == "on":
+            ws["f"] = B.tt_sort_trigger_slice(d_in, d_out, None, seg, runs, geo, prm, d_flags, d_seeds, d_ns, d_st, ws.get("f"))
+        else:
+            ws["s"] = B.tt_sort_slice(d_in, d_out, None, seg, runs, d_st, ws.get("s"))
+            ws["t"] = B.tt_trigger_slice(d_out, seg, geo, prm, d_flags, d_seeds, d_ns, d_st, ws.get("t"))
         ws["e"] = B.tt_extract_events(d_out, seg, d_seeds, d_ns, prm, d_ev, d_ne, d_flags, None, None, d_st, ws.get("e"))
 
     def barrier():
@@ -467,6 +470,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--graph", default="auto", choices=["auto", "on", "off"],
                     help="replay the step as a CUDA graph in the timed region (auto: yes, direct launches if capture fails)")
+    ap.add_argument("--fused", default="on", choices=["on", "off"],
+                    help="on: tt_sort_trigger_slice (L1 fused into the last merge level); off: the three separate calls")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     args = ap.parse_args()

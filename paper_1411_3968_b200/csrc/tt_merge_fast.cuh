@@ -22,8 +22,8 @@ static_assert(kFCap <= 4096, "12-bit element ids / bucket ids");
 
 struct FastSmem {
     uint4 tile[kFCap];               // staged run-major by TMA, then the sorted tile (in place)        64 KB
-    uint32_t cs[kFCap];              // buckets: count, then start << 16 | count; later relative times  16 KB
-    uint32_t list[kFCap];            // bucket members (composites); later perm values / floor|pmt      16 KB
+    uint32_t cs[kFCap + 4];          // buckets: count, then start << 16 | count; later relative times + 4 sentinels
+    uint32_t list[kFCap + 4];        // bucket members (composites); later perm values / floor|pmt (+ 4 readable)
     uint32_t fl[kFCap / 4 + 8];      // kFuse: flag bytes, shifted so that 16-byte groups match the global array
     uint32_t segstart[kMaxFan + 1];  // tile-local start of every run piece
     uint32_t cur[kMaxFan];           // absolute index of the first hit of every piece
@@ -32,7 +32,7 @@ struct FastSmem {
     uint64_t mbar;
 };
 static_assert(2 * (sizeof(FastSmem) + 1024) <= 233472, "two CTAs per SM");
-static_assert(offsetof(FastSmem, fl) % 16 == 0 && offsetof(FastSmem, cs) % 16 == 0, "16-byte accesses");
+static_assert(offsetof(FastSmem, fl) % 16 == 0 && offsetof(FastSmem, cs) % 16 == 0 && offsetof(FastSmem, list) % 16 == 0, "16-byte accesses");
 static_assert(kFItems == 8, "the bucket scan reads two uint4 per thread");
 
 __device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
@@ -41,6 +41,11 @@ __device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t by
     asm volatile("cp.async.bulk.commit_group;" ::: "memory");
 }
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+
+__device__ __forceinline__ uint64_t tile_key(const uint4* tile, uint32_t e) {
+    const uint2 v = *reinterpret_cast<const uint2*>(&tile[e]);
+    return (((uint64_t)v.y << 32) | v.x) ^ 0x8000000000000000ull;
+}
 
 template <bool kPerm, bool kFuse>
 __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, const uint4* __restrict__ in,
@@ -84,13 +89,16 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, c
         }
         return;
     }
+    // fused L1 needs the window to end inside 32-bit offsets from Ta: lc + width < 2^32.  A wider window (far wider
+    // than a tile anyway) leaves all L1 bits of the tile to l1_boundary_kernel's exact scans.
+    const bool l1_here = kFuse && fz.lc < 0xFFFFFFFFull - (uint32_t)DT;
     if (tid < K) {
         sm.segstart[tid] = my_s0;
         if (my_len) atomicOr(&sm.pstart[my_s0 >> 5], 1u << (my_s0 & 31u));
     }
     if (tid == 0) {
         sm.segstart[K] = total;
-        if (kFuse) lv.tile_open[blockIdx.x] = 0;
+        if (kFuse) lv.tile_open[blockIdx.x] = l1_here ? 0 : 1;
         mbar_expect_tx(&sm.mbar, total * 16u);
     }
     __syncthreads();
@@ -112,38 +120,34 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, c
     uint32_t fb[kFItems];    // composite high part (20 bits) << 12 | bucket
     uint32_t slot[kFItems];  // arrival position in the bucket, later start << 16 | count of the bucket
     bool unsorted = false;
+    if (check_runs && tid > 0 && tid < (uint32_t)kFCap / 32) {
+        // order across the 32-element groups of the loop below (its shuffle compares inside a group only): element
+        // 32 tid against its staged predecessor, unless it starts a piece
+        const uint32_t e = 32u * tid;
+        if (e < total && !(sm.pstart[tid] & 1u) && tile_key(sm.tile, e - 1) > tile_key(sm.tile, e)) unsorted = true;
+    }
 #pragma unroll
     for (int i = 0; i < kFItems; ++i) {
         const uint32_t e = tid + i * kFThreads;
         const bool in_tile = e < total;
-        uint32_t d = 0;
-        bool oob = false;
-        if (in_tile) {
-            const uint2 v = *reinterpret_cast<const uint2*>(&sm.tile[e]);
-            const uint32_t hi = (v.y ^ 0x80000000u) - Ta_hi - (v.x < Ta_lo ? 1u : 0u);  // high word of key - Ta
-            d = v.x - Ta_lo;
-            oob = hi != 0u || d >= width;  // only with unsorted runs (the splits assume sorted runs)
-            if (oob) d = (hi & 0x80000000u) ? 0u : width - 1u;
-        }
+        // key - Ta as (hi, d); a hit outside [0, width) can only come from unsorted runs (the splits assume sorted
+        // runs): it is flagged, and its bucket is clamped so that the ranks stay a permutation of the tile
+        const uint2 v = *reinterpret_cast<const uint2*>(&sm.tile[in_tile ? e : 0u]);
+        const uint32_t d = v.x - Ta_lo;
+        const uint32_t hi = (v.y ^ 0x80000000u) - Ta_hi - (v.x < Ta_lo ? 1u : 0u);
+        bool bad = hi != 0u || d >= width;
         if (check_runs) {
-            // order inside a run piece: the offset of the staged predecessor (the lane below; lane 0 reads it)
-            uint32_t dp = __shfl_up_sync(0xffffffffu, d, 1);
-            if (lane == 0 && in_tile && e > 0) {
-                const uint2 u = *reinterpret_cast<const uint2*>(&sm.tile[e - 1]);
-                const uint32_t hu = (u.y ^ 0x80000000u) - Ta_hi - (u.x < Ta_lo ? 1u : 0u);
-                dp = hu ? ((hu & 0x80000000u) ? 0u : 0xFFFFFFFFu) : u.x - Ta_lo;
-            }
-            const uint32_t ps = sm.pstart[e >> 5];  // one word per warp: a broadcast
-            if (in_tile && e > 0 && !((ps >> lane) & 1u) && dp > d) unsorted = true;
+            // order inside a run piece: the offset of the staged predecessor = the lane below
+            const uint32_t dp = __shfl_up_sync(0xffffffffu, d, 1);
+            const uint32_t ps = sm.pstart[(tid >> 5) + i * (kFThreads / 32)];  // one word per warp: a broadcast
+            bad |= lane != 0u && !((ps >> lane) & 1u) && dp > d;
         }
-        unsorted |= oob;
-        fb[i] = 0; slot[i] = 0;
-        if (in_tile) {
-            const uint64_t pr = (uint64_t)d * scale;
-            const uint32_t b = (uint32_t)(pr >> 32);
-            slot[i] = atomicAdd(&sm.cs[b], 1u);
-            fb[i] = ((uint32_t)pr & 0xFFFFF000u) | b;
-        }
+        unsorted |= in_tile && bad;
+        const uint64_t pr = (uint64_t)d * scale;
+        const uint32_t b = min((uint32_t)(pr >> 32), (uint32_t)kFCap - 1u);
+        fb[i] = ((uint32_t)pr & 0xFFFFF000u) | b;
+        slot[i] = 0;
+        if (in_tile) slot[i] = atomicAdd(&sm.cs[b], 1u);
     }
     if (__syncthreads_or(unsorted) && tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
     // ---- exclusive scan of the bucket counts: kFItems consecutive buckets per thread -> start << 16 | count
@@ -166,28 +170,28 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, c
 #pragma unroll
     for (int i = 0; i < kFItems; ++i) {
         const uint32_t e = tid + i * kFThreads;
-        if (e < total) {
-            const uint32_t w = sm.cs[fb[i] & 0xFFFu];
-            if ((w & 0xFFFFu) > 1u) sm.list[(w >> 16) + slot[i]] = (fb[i] & 0xFFFFF000u) | e;
-            slot[i] = w;
-        }
+        // (slots past the tile's end read bucket fb = garbage & 0xFFF: in range, and their cb/rank are never used)
+        const uint32_t w = sm.cs[fb[i] & 0xFFFu];
+        if (e < total && (w & 0xFFFFu) > 1u) sm.list[(w >> 16) + slot[i]] = (fb[i] & 0xFFFFF000u) | e;
+        slot[i] = e < total ? w : 0u;
     }
     __syncthreads();
-    // ---- rank = bucket start + members of the bucket that order before this hit
+    // ---- rank = bucket start + members of the bucket that order before this hit (four in a straight line: 99 % of
+    // the hits at a bucket load of 0.875; the loop is for the rare fuller buckets)
     uint32_t rk[kFItems];
 #pragma unroll
     for (int i = 0; i < kFItems; ++i) {
         const uint32_t e = tid + i * kFThreads;
         const uint32_t s0 = slot[i] >> 16, cb = slot[i] & 0xFFFFu;
+        const uint32_t c = (fb[i] & 0xFFFFF000u) | e;
         uint32_t r = s0;
-        if (e < total && cb > 1u) {
-            const uint32_t c = (fb[i] & 0xFFFFF000u) | e;
-#pragma unroll
-            for (uint32_t q = 0; q < 3u; ++q) {
-                const uint32_t o = q < cb ? sm.list[s0 + q] : 0xFFFFFFFFu;
-                r += o < c ? 1u : 0u;
-            }
-            for (uint32_t q = 3u; q < cb; ++q) r += sm.list[s0 + q] < c ? 1u : 0u;
+        if (cb > 1u) {
+            const uint32_t* const lp = sm.list + s0;
+            const uint32_t o0 = lp[0], o1 = lp[1];
+            const uint32_t o2 = cb > 2u ? lp[2] : 0xFFFFFFFFu, o3 = cb > 3u ? lp[3] : 0xFFFFFFFFu;
+            r += (o0 < c ? 1u : 0u) + (o1 < c ? 1u : 0u) + (o2 < c ? 1u : 0u) + (o3 < c ? 1u : 0u);
+#pragma unroll 1
+            for (uint32_t q = 4u; q < cb; ++q) r += lp[q] < c ? 1u : 0u;
         }
         rk[i] = r;
     }
@@ -205,7 +209,7 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, c
         if (e < total) sm.tile[rk[i]] = rec[i];
     }
     if (kPerm) {
-#pragma unroll 1
+#pragma unroll
         for (int i = 0; i < kFItems; ++i) {
             const uint32_t e = tid + i * kFThreads;
             if (e < total) {
@@ -224,40 +228,73 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, c
         for (uint32_t r = tid; r < n_store; r += kFThreads) perm_out[out_base + r] = sm.list[r];
         if (kFuse) __syncthreads();  // list is reused below
     }
-    if (kFuse) {
+    if (kFuse && l1_here) {
         // ---- L1 on the sorted tile.  cs[] <- time offset from Ta (exact in 32 bits: the tile spans < 2^32), list[] <-
         // floor << 16 | pmt, fl bytes <- Q.  Flag byte of tile hit r sits at byte sh + r, sh = the global address's
         // offset in its 16-byte group, so whole groups leave with 16-byte stores.
         uint8_t* const gfl = fz.flags + out_base;
         const uint32_t sh = (uint32_t)((uintptr_t)gfl & 15u);
         uint8_t* const fbytes = reinterpret_cast<uint8_t*>(sm.fl);
-        const uint32_t lc32 = fz.lc > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)fz.lc;
+        const uint32_t lc32 = (uint32_t)fz.lc;  // lc < 2^32 - width here (else the tile is left to the exact scans)
 #pragma unroll
         for (int i = 0; i < kFItems; ++i) {
             const uint32_t r = tid + i * kFThreads;
             if (r < total) {
                 const uint4 v = sm.tile[r];
-                sm.cs[r] = v.x - Ta_lo;
+                sm.cs[r] = min(v.x - Ta_lo, width - 1u);  // (the clamp only acts on unsorted input: the scans below end at the sentinels)
                 sm.list[r] = v.z;
                 fbytes[sh + r] = (v.w & 0xFFFFu) >= fz.q_thresh ? (uint8_t)TT_Q : (uint8_t)0;
             }
         }
+        if (tid < 4u) sm.cs[total + tid] = 0xFFFFFFFFu;  // sentinels: outside every window (offsets are < width)
         __syncthreads();
-#pragma unroll 1
-        for (int i = 0; i < kFItems; ++i) {
-            const uint32_t e = tid + i * kFThreads;
-            if (e >= total) break;
-            const uint32_t ti = sm.cs[e], ki = sm.list[e];
-            bool found = false;
-            for (uint32_t j = e + 1; j < total; ++j) {
-                if (sm.cs[j] - ti > lc32) break;
-                const uint32_t x = sm.list[j] ^ ki;
-                if (x - 1u < 0xFFFFu) {  // same floor (high half equal), other pmt (low half differs)
-                    found = true;
-                    atomicOr(&sm.fl[(sh + j) >> 2], (uint32_t)TT_LC << (8u * ((sh + j) & 3u)));
+        // Every hit scans FORWARD over the hits inside its window and marks both partners of a same-floor / other-PMT
+        // pair, so a pair is tested once.  Two loops, chosen per tile from its density (block-uniform):
+        //   sparse (under ~1.5 hits per window: one tower): one hit per step, the time test first -- most hits leave at once;
+        //   dense (many superimposed towers: ~9 hits ahead inside 20 ns): four hits per step, the floor filter first (a
+        //   same-floor hit among them is rare), the time test only on a match and for the loop condition.
+        if ((uint64_t)total * lc32 < (uint64_t)width + (width >> 1)) {
+#pragma unroll 2
+            for (int i = 0; i < kFItems; ++i) {
+                const uint32_t e = tid + i * kFThreads;
+                if (e >= total) break;
+                const uint32_t ti = sm.cs[e], ki = sm.list[e];
+                bool found = false;
+                for (uint32_t j = e + 1; sm.cs[j] - ti <= lc32; ++j) {  // ends at the sentinel
+                    const uint32_t x = sm.list[j] ^ ki;
+                    if (x - 1u < 0xFFFFu) {  // same floor (high half equal), other pmt (low half differs)
+                        found = true;
+                        atomicOr(&sm.fl[(sh + j) >> 2], (uint32_t)TT_LC << (8u * ((sh + j) & 3u)));
+                    }
                 }
+                if (found) atomicOr(&sm.fl[(sh + e) >> 2], (uint32_t)TT_LC << (8u * ((sh + e) & 3u)));
             }
-            if (found) atomicOr(&sm.fl[(sh + e) >> 2], (uint32_t)TT_LC << (8u * ((sh + e) & 3u)));
+        } else {
+#pragma unroll 2
+            for (int i = 0; i < kFItems; ++i) {
+                const uint32_t e = tid + i * kFThreads;
+                if (e >= total) break;
+                const uint32_t ti = sm.cs[e], ki = sm.list[e];
+                bool found = false;
+                uint32_t j = e + 1;
+                bool more;
+                do {
+                    const uint32_t x0 = sm.list[j] ^ ki, x1 = sm.list[j + 1] ^ ki, x2 = sm.list[j + 2] ^ ki, x3 = sm.list[j + 3] ^ ki;
+                    more = sm.cs[j + 3] - ti <= lc32;
+                    if ((x0 - 1u < 0xFFFFu) | (x1 - 1u < 0xFFFFu) | (x2 - 1u < 0xFFFFu) | (x3 - 1u < 0xFFFFu)) {
+                        const uint32_t xs[4] = {x0, x1, x2, x3};
+#pragma unroll
+                        for (uint32_t q = 0; q < 4u; ++q) {
+                            if (xs[q] - 1u < 0xFFFFu && sm.cs[j + q] - ti <= lc32) {
+                                found = true;
+                                atomicOr(&sm.fl[(sh + j + q) >> 2], (uint32_t)TT_LC << (8u * ((sh + j + q) & 3u)));
+                            }
+                        }
+                    }
+                    j += 4;
+                } while (more);
+                if (found) atomicOr(&sm.fl[(sh + e) >> 2], (uint32_t)TT_LC << (8u * ((sh + e) & 3u)));
+            }
         }
         __syncthreads();
         // flags out: L1 = Q | LC
