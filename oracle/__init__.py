@@ -178,3 +178,23 @@ def l0_dntw(sorted_hits: np.ndarray, seg_offsets: np.ndarray, *, multiplicity: i
     if rc != 0:
         raise ValueError("oracle_l0_dntw: invalid parameters")
     return l0, ns.value
+
+
+RAW = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("n_samples", "<u2"), ("pad", "<u2")])
+
+
+def prepare(raw: np.ndarray, samples: np.ndarray, slice_offsets: np.ndarray, n_pmt: int):
+    """The paper's CPU preparation (R24): raw headers + concatenated waveforms ->
+    (fixed-size hit records slice-major / PMT-major, run offsets [n_slices * n_pmt + 1], status)."""
+    r = np.ascontiguousarray(raw, dtype=RAW)
+    sm = np.ascontiguousarray(samples, dtype=np.uint16)
+    so = np.ascontiguousarray(slice_offsets, dtype=np.uint32)
+    n, ns = r.shape[0], len(so) - 1
+    out = np.zeros(n, dtype=HIT)
+    runs = np.zeros(ns * int(n_pmt) + 1, dtype=np.uint32)
+    st = ctypes.c_int32(0)
+    rc = lib().oracle_prepare(_p(r), _p(sm), ctypes.c_uint32(n), ctypes.c_uint32(len(sm)), _p(so), ctypes.c_uint32(ns),
+                              ctypes.c_uint32(int(n_pmt)), _p(out), _p(runs), ctypes.byref(st))
+    if rc != 0:
+        raise ValueError("oracle_prepare: invalid parameters")
+    return out, runs, st.value

@@ -28,6 +28,11 @@
 //                   (used first, "as level 0 trigger").  DESIGN.md reading R14: the printed formula has the
 //                   sign reversed and 7 hits span i..i+6, so the test is t[k+N-1] - t[k] < TW, strict as printed.
 //
+//   oracle_prepare  PAPER.md:41 ("the raw hits are converted to a fixed size structure": charge, time, DU id),
+//                   PAPER.md:45 (five 200 ms slices packed into one buffer at offsets), PAPER.md:23 (each PMT's
+//                   stream is time-ordered, the merged stream is not PMT-major).  DESIGN.md reading R24 (the raw
+//                   format is this build's: the paper gives none).
+//
 // Pins (tests/test_oracle_*.py, -m "not gpu"): brute-force pair / subset enumeration written
 // separately in oracle/brute.py, numpy stable argsort, Poisson closed forms, N-in-TW special
 // case, interval-union brute force, hand-written boundary cases.  No function
@@ -339,6 +344,53 @@ int oracle_l0_dntw(const Hit* h, uint32_t n, const uint32_t* seg_off, uint32_t n
         }
     }
     *n_start = count;
+    return 0;
+}
+
+// ---- NEXT-3: the paper's CPU preparation.  Raw hit k = a 16-byte header {t_ps, pmt_id, floor,
+// n_samples, pad} and n_samples 16-bit waveform samples; the waveforms of all hits are concatenated in hit order, so
+// hit k's samples start at the sum of the sample counts before it.  charge = sum of the samples, saturated at 65535;
+// samples that would lie behind the waveform section count as 0 and set status bit 32.  Output: fixed-size records,
+// slice-major then PMT-major, arrival order kept inside a (slice, PMT) run; run_off[slice * n_pmt + pmt] .. =
+// offsets of the runs.  A hit with pmt_id >= n_pmt sets status bit 8 and is filed under the last PMT of its slice.
+struct RawHit {
+    int64_t t_ps;
+    uint16_t pmt_id, floor, n_samples, pad;
+};
+static_assert(sizeof(RawHit) == 16, "raw header is 16 bytes");
+
+int oracle_prepare(const RawHit* raw, const uint16_t* samples, uint32_t n_raw, uint32_t n_samples_total,
+                   const uint32_t* slice_off, uint32_t n_slices, uint32_t n_pmt, Hit* out, uint32_t* run_off,
+                   int32_t* status) {
+    if (n_pmt < 1 || n_slices < 1) return -1;
+    *status = 0;
+    // waveform start of every hit
+    std::vector<uint64_t> woff(n_raw + 1, 0);
+    for (uint32_t k = 0; k < n_raw; ++k) woff[k + 1] = woff[k] + raw[k].n_samples;
+    uint32_t pos = 0;
+    for (uint32_t s = 0; s < n_slices; ++s)
+        for (uint32_t p = 0; p < n_pmt; ++p) {
+            run_off[(uint64_t)s * n_pmt + p] = pos;
+            for (uint32_t k = slice_off[s]; k < slice_off[s + 1]; ++k) {
+                uint32_t q = raw[k].pmt_id;
+                if (q >= n_pmt) { *status |= 8; q = n_pmt - 1; }
+                if (q != p) continue;
+                uint64_t sum = 0;
+                for (uint32_t j = 0; j < raw[k].n_samples; ++j) {
+                    const uint64_t at = woff[k] + j;
+                    if (at >= n_samples_total) { *status |= 32; continue; }
+                    sum += samples[at];
+                }
+                Hit h;
+                h.t_ps = raw[k].t_ps;
+                h.pmt_id = raw[k].pmt_id;
+                h.floor = raw[k].floor;
+                h.charge = (uint16_t)(sum > 65535 ? 65535 : sum);
+                h.pad = raw[k].pad;
+                out[pos++] = h;
+            }
+        }
+    run_off[(uint64_t)n_slices * n_pmt] = pos;
     return 0;
 }
 

@@ -312,3 +312,49 @@ def shuffled(w: Workload, seed: int = 7) -> tuple[np.ndarray, np.ndarray]:
         out[a:b] = w.hits[p]
         perm[a:b] = p
     return out, perm
+
+
+RAW_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("n_samples", "<u2"), ("pad", "<u2")])
+
+
+def make_raw(w: Workload, frame_ps: int = 100_000_000, seed: int = 11):
+    """The workload as the RAW stream the paper's preparation step starts from ("a header with the GPS
+    time and geometry information, followed by a sampled charge waveform with a variable size"; 28 bytes on average,
+    PAPER.md:21).  Synthetic format (R24): 16-byte headers in ARRIVAL order + all waveforms concatenated in
+    the same order.  Arrival order inside a slice: frame by frame (frame = t // frame_ps, the Hit Manager merging the
+    PMT streams), PMT by PMT inside a frame, so every PMT's hits stay time-ordered but the stream is not
+    PMT-major.  A slice = n_pmt consecutive runs of the workload (a 200 ms sub-slice of one tower or tower array).
+    The waveform of a hit has 1 + Poisson(5) samples (16 + 2 * 6 = 28 bytes per hit on average) that sum to its charge.
+    Returns (raw headers, samples uint16, slice_offsets uint32)."""
+    P = w.geometry.n_pmt
+    n_runs = len(w.run_offsets) - 1
+    assert n_runs % P == 0, "runs are (slice, PMT)"
+    n_slices = n_runs // P
+    slice_off = np.asarray(w.run_offsets[::P], dtype=np.uint32)
+    assert len(slice_off) == n_slices + 1
+    h = w.hits
+    n = w.n
+    slice_id = np.repeat(np.arange(n_slices, dtype=np.int64), np.diff(slice_off.astype(np.int64)))
+    frame = h["t_ps"] // frame_ps
+    # stable: inside (slice, frame, pmt) the workload's order (= time order of that PMT) is kept
+    order = np.lexsort((h["pmt_id"], frame, slice_id))
+    ha = h[order]
+    rng = np.random.default_rng(seed)
+    ns = (1 + rng.poisson(5.0, size=n)).astype(np.uint16)
+    raw = np.zeros(n, dtype=RAW_DTYPE)
+    raw["t_ps"], raw["pmt_id"], raw["floor"], raw["pad"], raw["n_samples"] = ha["t_ps"], ha["pmt_id"], ha["floor"], ha["pad"], ns
+    # pulse shape: sample j of a waveform of m samples gets floor(charge * wgt_j), wgt ~ a fixed falling shape; what
+    # the floors lose goes to sample 0, so the samples sum to the charge exactly
+    woff = np.zeros(n + 1, dtype=np.int64)
+    np.cumsum(ns, out=woff[1:])
+    total = int(woff[-1])
+    hit_of = np.repeat(np.arange(n, dtype=np.int64), ns)
+    j = np.arange(total, dtype=np.int64) - woff[hit_of]
+    m = ns[hit_of].astype(np.float64)
+    wgt = (m - j) / (m * (m + 1) / 2.0)  # m, m-1, ..., 1 over their sum
+    c = ha["charge"].astype(np.int64)
+    samples = np.floor(c[hit_of] * wgt).astype(np.int64)
+    lost = c - np.bincount(hit_of, weights=samples, minlength=n).astype(np.int64)
+    samples[woff[:-1]] += lost
+    assert samples.min() >= 0 and samples.max() <= 65535
+    return raw, samples.astype(np.uint16), slice_off
