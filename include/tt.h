@@ -14,6 +14,8 @@
  *   tt_l0_dntw         PAPER.md:60 (DN7TW1000: N hits from different PMTs in TW)   -- distinct-PMT level-0 trigger
  *   tt_pair_seeds      PAPER.md:61-63 (SC, FC, AFC coincidences)          -- the paper's pair seeds
  *   tt_l0_combine      PAPER.md:65, 73 (N7TW with [SC and AFC] or [FC and AFC]) -- the paper's combined trigger
+ *   tt_prepare_slice   PAPER.md:41-47 (raw hits -> fixed-size records, slices packed into one buffer) -- preparation
+ *   tt_sort_trigger_slice  tt_sort_slice + tt_trigger_slice as one call, L1 fused into the last merge level
  *
  * Conventions
  *   d_*   device pointers (caller-owned; the library never allocates in the three hot calls)
@@ -79,6 +81,7 @@ enum {
     TT_S_EVENT_OVERFLOW = 2, /* likewise for events                                                   */
     TT_S_RUN_UNSORTED = 4,   /* a run given by d_run_offsets is not non-decreasing: output unspecified */
     TT_S_BAD_PMT = 8,        /* an L1 hit has pmt_id >= n_pmt (it has no L2 edges)                     */
+    TT_S_RAW_TRUNCATED = 32, /* tt_prepare_slice: a waveform reaches behind the sample section (missing samples = 0) */
     TT_S_DENSITY = 16        /* an L1 hit has more than TT_MAX_NEIGHBOURS L1 hits of its segment within
                                 +-min(W, largest table entry) of it: its L2STAR bit is exact, and its
                                 clique-mode L2 bit is SET FROM the L2STAR bit (fail open: a superset of
@@ -197,6 +200,28 @@ int tt_pair_seeds(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offs
  * number of CAND_A and of CAND_B starts. */
 int tt_l0_combine(const uint8_t* d_l0, const uint8_t* d_pair_bits, uint32_t n, uint32_t multiplicity,
                   uint8_t* d_cand, uint32_t* d_n_cand, void* stream);
+
+/* The paper's preparation step on the GPU ("the raw hits are converted to a fixed
+ * size structure", PAPER.md:45 five 200 ms slices packed into one buffer at offsets: 200-300 ms of CPU
+ * time per second of data in the paper).  The paper does not give its raw format; this build's (reading R24):
+ *   d_raw[n_raw]     16-byte headers in ARRIVAL order: every PMT's hits time-ordered, the PMTs interleaved
+ *   d_samples[...]   the sampled charge waveforms of all hits, concatenated in the same order, uint16 each; hit k owns
+ *                    n_samples_k samples starting at the sum of the sample counts before it (< 2^32 in total)
+ *   d_slice_offsets  [n_slices + 1] (device; h_slice_offsets = the same on the host) cut d_raw into 200 ms slices
+ * Output: d_out[n_raw] fixed-size records {t_ps, pmt_id, floor, charge = min(65535, sum of the samples), pad} ordered
+ * slice-major, then PMT-major, arrival order kept inside a (slice, PMT) run -- the concatenated, individually
+ * time-ordered runs tt_sort_slice takes -- and d_run_offsets[n_slices * n_pmt + 1] (device), their offsets.  (The host
+ * copy tt_sort_slice also wants is a 4-byte-per-run read-back by the caller.)  n_raw > out_cap (the buffer the caller
+ * sized: for 5 x the nominal rate) returns TT_E_INVAL.  Status bits: TT_S_BAD_PMT (pmt_id >= n_pmt: the
+ * hit is filed under the last PMT of its slice, record unchanged), TT_S_RAW_TRUNCATED.  Asynchronous on `stream`. */
+typedef struct {
+    int64_t t_ps;
+    uint16_t pmt_id, floor, n_samples, pad;
+} tt_raw_hit;
+int tt_prepare_slice(const tt_raw_hit* d_raw, const uint16_t* d_samples, uint32_t n_raw, uint32_t n_samples_total,
+                     const uint32_t* d_slice_offsets, const uint32_t* h_slice_offsets, uint32_t n_slices,
+                     uint32_t n_pmt, tt_hit* d_out, uint32_t out_cap, uint32_t* d_run_offsets, void* d_ws,
+                     size_t* ws_bytes, int32_t* d_status, void* stream);
 
 /* Whole-slice convenience with HOST buffers (end-to-end use and timing; not a hot call).
  * tt_host_ctx_create allocates, once, device buffers and workspaces for slices of up to max_n hits,

@@ -20,11 +20,12 @@ c_u32, c_i32, c_vp, c_sz = ctypes.c_uint32, ctypes.c_int32, ctypes.c_void_p, cty
 TT_Q, TT_LC, TT_L1, TT_L2STAR, TT_L2, TT_INEVT = 1, 2, 4, 8, 16, 32
 TT_OK, TT_E_INVAL, TT_E_CUDA, TT_E_WORKSPACE = 0, -1, -2, -3
 TT_S_SEED_OVERFLOW, TT_S_EVENT_OVERFLOW, TT_S_RUN_UNSORTED, TT_S_BAD_PMT, TT_S_DENSITY = 1, 2, 4, 8, 16
+TT_S_RAW_TRUNCATED = 32
 
 EXPORTS = ["tt_version", "tt_geometry_create", "tt_geometry_destroy", "tt_sort_slice", "tt_trigger_slice",
            "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host", "tt_launch_count",
            "tt_prof_enable", "tt_prof_read", "tt_l0_ntw", "tt_pair_seeds", "tt_l0_combine",
-           "tt_l0_dntw", "tt_sort_trigger_slice"]
+           "tt_l0_dntw", "tt_sort_trigger_slice", "tt_prepare_slice"]
 
 HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
 EVENT_DTYPE = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
@@ -261,6 +262,46 @@ def tt_extract_events(d_sorted: torch.Tensor, seg: Offsets, d_seeds: torch.Tenso
     nb = c_sz(ws.numel())
     _check(call(_dp(ws), ctypes.byref(nb)), "tt_extract_events")
     return ws
+
+
+RAW_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("n_samples", "<u2"), ("pad", "<u2")])
+
+
+def tt_prepare_slice(d_raw: torch.Tensor, d_samples: torch.Tensor, slices: Offsets, n_pmt: int, d_out: torch.Tensor,
+                     d_run_offsets: torch.Tensor, d_status: torch.Tensor, ws: torch.Tensor | None = None) -> torch.Tensor:
+    """Enqueue tt_prepare_slice: raw headers (n, 2) int64 + waveform samples (int16 storage of uint16)
+    -> d_out (n, 2) int64 PMT-major records and d_run_offsets int32[n_slices * n_pmt + 1]."""
+    _need_cuda()
+    L = load()
+    n = d_raw.shape[0]
+    assert d_samples.dtype in (torch.int16, torch.uint16) and d_run_offsets.numel() >= slices.count * n_pmt + 1
+
+    def call(wsp, nbytes):
+        return L.tt_prepare_slice(_dp(d_raw), _dp(d_samples), c_u32(n), c_u32(d_samples.numel()), _dp(slices.d),
+                                  _hp(slices.h), c_u32(slices.count), c_u32(int(n_pmt)), _dp(d_out), c_u32(d_out.shape[0]),
+                                  _dp(d_run_offsets), wsp, nbytes, _dp(d_status), _stream())
+
+    if ws is None:
+        ws = _ws(call, "tt_prepare_slice")
+    nb = c_sz(ws.numel())
+    _check(call(_dp(ws), ctypes.byref(nb)), "tt_prepare_slice")
+    return ws
+
+
+def prepare_slice(raw: np.ndarray, samples: np.ndarray, slice_offsets, n_pmt: int):
+    """Host-array convenience around tt_prepare_slice -> (records, run offsets, status)."""
+    _need_cuda()
+    r = np.ascontiguousarray(raw, dtype=RAW_DTYPE)
+    n = len(r)
+    d_raw = torch.from_numpy(r.view(np.int64).reshape(-1, 2).copy()).cuda()
+    d_samples = torch.from_numpy(np.ascontiguousarray(samples, dtype=np.uint16).view(np.int16).copy()).cuda()
+    sl = Offsets(slice_offsets)
+    d_out = torch.full((max(n, 1), 2), -1, dtype=torch.int64, device="cuda")[:n]
+    d_runs = torch.full((sl.count * n_pmt + 1,), -1, dtype=torch.int32, device="cuda")
+    d_st = torch.zeros(1, dtype=torch.int32, device="cuda")
+    tt_prepare_slice(d_raw, d_samples, sl, n_pmt, d_out, d_runs, d_st)
+    torch.cuda.synchronize()
+    return hits_to_host(d_out) if n else np.zeros(0, dtype=HIT_DTYPE), d_runs.cpu().numpy().view(np.uint32), int(d_st.item())
 
 
 TT_L0_START, TT_L0_MEMBER = 1, 2

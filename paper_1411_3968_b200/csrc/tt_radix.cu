@@ -7,7 +7,7 @@
 // Segments: after the 8 key passes, ceil(log256(n_seg)) more passes on the segment id of the input
 // index make every segment contiguous again (LSD: the last digit dominates), sorted inside.
 // Passes whose digit is the same for all elements are skipped (decided on the device).
-#include "tt_common.cuh"
+#include "tt_radix.cuh"
 
 namespace tt {
 
@@ -15,11 +15,6 @@ constexpr int kRThreads = 256;
 constexpr int kRItems = 8;
 constexpr int kRTile = kRThreads * kRItems;  // 2048
 constexpr int kRChunks = kRItems * (kRThreads / 32);  // 64 warp-chunks of 32 elements per tile
-
-struct RadixState {        // device-resident control block
-    uint32_t cur;          // which ping-pong buffer holds the current pairs (0/1)
-    uint32_t skip;         // set by the scan step of a pass whose digit is constant
-};
 
 __global__ void __launch_bounds__(256) radix_extract_kernel(const uint4* __restrict__ hits, uint64_t* __restrict__ keys,
                                                             uint32_t* __restrict__ idx, uint32_t n,
@@ -145,14 +140,7 @@ __global__ void __launch_bounds__(256) radix_gather_kernel(const uint4* __restri
     if (perm) perm[i] = src;
 }
 
-struct RadixPlan {
-    uint64_t *keys0, *keys1;
-    uint32_t *idx0, *idx1, *hist, *scan_scratch;
-    RadixState* st;
-    uint32_t nblocks;
-};
-
-static void radix_plan(Arena& a, uint32_t n, RadixPlan& p) {
+void radix_plan(Arena& a, uint32_t n, RadixPlan& p) {
     p.nblocks = div_up(n, kRTile);
     p.keys0 = a.take<uint64_t>(n);
     p.keys1 = a.take<uint64_t>(n);
@@ -161,6 +149,25 @@ static void radix_plan(Arena& a, uint32_t n, RadixPlan& p) {
     p.hist = a.take<uint32_t>((size_t)256 * p.nblocks);
     p.scan_scratch = a.take<uint32_t>(scan_ws_count(256u * p.nblocks));
     p.st = a.take<RadixState>(1);
+}
+
+// LSD passes [pass_begin, pass_end) over the (key, index) pairs of the plan; st->cur says where they end up
+int radix_run_passes(const RadixPlan& p, uint32_t n, int pass_begin, int pass_end, const uint32_t* d_seg_offsets,
+                     uint32_t n_seg, cudaStream_t s) {
+    for (int pass = pass_begin; pass < pass_end; ++pass) {
+        prof_mark(s, "sort.radix_hist");
+        TT_K(radix_hist_kernel)<<<p.nblocks, kRThreads, 0, s>>>(p.keys0, p.keys1, p.idx0, p.idx1, n, pass, d_seg_offsets,
+                                                          n_seg, p.st, p.hist, p.nblocks);
+        prof_mark(s, "sort.radix_scan");
+        int rc = exclusive_scan_u32(p.hist, p.hist, 256u * p.nblocks, p.scan_scratch, nullptr, s);
+        if (rc != TT_OK) return rc;
+        TT_K(radix_decide_kernel)<<<1, 256, 0, s>>>(p.hist, p.nblocks, n, p.st);
+        prof_mark(s, "sort.radix_scatter");
+        TT_K(radix_scatter_kernel)<<<p.nblocks, kRThreads, 0, s>>>(p.keys0, p.keys1, p.idx0, p.idx1, n, pass,
+                                                             d_seg_offsets, n_seg, p.st, p.hist, p.nblocks);
+        TT_K(radix_flip_kernel)<<<1, 1, 0, s>>>(p.st);
+    }
+    return TT_OK;
 }
 
 size_t radix_ws_bytes(uint32_t n) {
@@ -181,19 +188,8 @@ int radix_sort(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, 
     TT_K(radix_extract_kernel)<<<nb256, 256, 0, s>>>((const uint4*)d_in, p.keys0, p.idx0, n, p.st);
     int seg_passes = 0;
     for (uint32_t v = n_seg - 1; v; v >>= 8) ++seg_passes;
-    for (int pass = 0; pass < 8 + seg_passes; ++pass) {
-        prof_mark(s, "sort.radix_hist");
-        TT_K(radix_hist_kernel)<<<p.nblocks, kRThreads, 0, s>>>(p.keys0, p.keys1, p.idx0, p.idx1, n, pass, d_seg_offsets,
-                                                          n_seg, p.st, p.hist, p.nblocks);
-        prof_mark(s, "sort.radix_scan");
-        int rc = exclusive_scan_u32(p.hist, p.hist, 256u * p.nblocks, p.scan_scratch, nullptr, s);
-        if (rc != TT_OK) return rc;
-        TT_K(radix_decide_kernel)<<<1, 256, 0, s>>>(p.hist, p.nblocks, n, p.st);
-        prof_mark(s, "sort.radix_scatter");
-        TT_K(radix_scatter_kernel)<<<p.nblocks, kRThreads, 0, s>>>(p.keys0, p.keys1, p.idx0, p.idx1, n, pass,
-                                                             d_seg_offsets, n_seg, p.st, p.hist, p.nblocks);
-        TT_K(radix_flip_kernel)<<<1, 1, 0, s>>>(p.st);
-    }
+    const int rc = radix_run_passes(p, n, 0, 8 + seg_passes, d_seg_offsets, n_seg, s);
+    if (rc != TT_OK) return rc;
     prof_mark(s, "sort.radix_gather");
     TT_K(radix_gather_kernel)<<<nb256, 256, 0, s>>>((const uint4*)d_in, (uint4*)d_out, d_perm, p.idx0, p.idx1, p.st, n);
     prof_end(s);
