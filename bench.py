@@ -191,6 +191,226 @@ def run_reference(args):
     }))
 
 
+def time_oracle_all_cores(cfg: int):
+    """the oracle on ALL host cores where the split is exact -- independent segments (cfg3), else time
+    chunks with a 6.02 us halo (chunking invariance P12) -- each chunk through sort -> trigger -> events in its own
+    thread (the C++ oracle releases the GIL).  Same bounded sample as the single-core figure."""
+    import oracle
+    from concurrent.futures import ThreadPoolExecutor
+    from paper_1411_3968_b200 import workload as W
+
+    ts, ss = ORACLE_SAMPLE[cfg]
+    w = W.make_config(cfg, time_scale=ts, seg_scale=ss)
+    g, p = w.geometry, w.params
+    cores = os.cpu_count() or 1
+    halo = p.event_half_ps + p.l2_window_ps + p.lc_window_ps
+    seg = np.asarray(w.seg_offsets, dtype=np.int64)
+    chunks = []
+    if len(seg) - 1 >= cores:
+        for s in range(len(seg) - 1):
+            chunks.append(np.ascontiguousarray(w.hits[seg[s]:seg[s + 1]]))
+        how = f"{len(chunks)} independent segments"
+    else:
+        t = w.hits["t_ps"]
+        lo, hi = int(t.min()), int(t.max()) + 1
+        nch = cores * 2
+        edges = np.linspace(lo, hi, nch + 1).astype(np.int64)
+        for k in range(nch):
+            sel = (t >= edges[k] - halo) & (t < edges[k + 1] + halo)
+            chunks.append(np.ascontiguousarray(w.hits[sel]))  # input order = run-major: the oracle's stable order
+        how = f"{nch} time chunks with a {halo} ps halo each side (the halo hits are processed twice)"
+    oracle.build()
+
+    def work(h):
+        so = np.array([0, len(h)], dtype=np.uint32)
+        srt, _ = oracle.sort(h, so)
+        tr = oracle.trigger(srt, so, g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks, q_thresh=p.q_thresh,
+                            lc_window_ps=p.lc_window_ps, l2_window_ps=p.l2_window_ps, l2_multiplicity=p.l2_multiplicity,
+                            l2_mode=p.l2_mode, event_half_ps=p.event_half_ps)
+        fl = tr.flags.copy()
+        oracle.events(srt, so, tr.seeds, event_half_ps=p.event_half_ps, flags=fl)
+        return len(tr.seeds)
+
+    t0 = time.perf_counter()
+    with ThreadPoolExecutor(max_workers=cores) as ex:
+        list(ex.map(work, chunks))
+    dt = time.perf_counter() - t0
+    return {"value": w.n / dt, "unit": "hits/s", "cores": cores, "kind": "oracle", "split": how,
+            "sample": f"cfg{cfg} at time_scale={ts}, seg_scale={ss}: {w.n} hits in {1e3 * dt:.0f} ms"}
+
+
+def _cuda_time(fn, reps):
+    import torch
+
+    fn()
+    torch.cuda.synchronize()
+    b0, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    b0.record()
+    for _ in range(reps):
+        fn()
+    b1.record()
+    torch.cuda.synchronize()
+    return b0.elapsed_time(b1) / reps
+
+
+def time_radix(B, run, peak):
+    """tt_sort_slice with run_offsets = NULL (arbitrary input: the LSD radix path) on this run's hits."""
+    import torch
+
+    st = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ws = {}
+
+    def go():
+        ws["r"] = B.tt_sort_slice(run.d_in, run.d_out, None, run.seg, None, st, ws.get("r"))
+
+    ms = _cuda_time(go, 3)
+    return {"workload": run.w.name, "hits": run.n, "ms": ms, "hits_per_s": run.n / (ms * 1e-3),
+            "alg_bytes_per_hit": 32, "frac": 32.0 * run.n / (ms * 1e-3) / 1e9 / peak,
+            "note": "8-bit LSD passes over the varying key bits + one gather: ~5 passes x (12 B read + 24 B moved)"}
+
+
+def time_prepare(B, peak):
+    """tt_prepare_slice (NEXT-3) on the raw stream of a cfg2-shaped burst: five 200 ms sub-slices at
+    one tenth of the duration (3 M raw hits, 28 B each on average) -> PMT-major 16-byte records + run offsets."""
+    import torch
+
+    from paper_1411_3968_b200 import workload as W
+
+    w = W.make_config(2, time_scale=0.1)
+    raw, samples, slice_off = W.make_raw(w)
+    n = len(raw)
+    d_raw = torch.from_numpy(raw.view(np.int64).reshape(-1, 2).copy()).cuda()
+    d_samples = torch.from_numpy(samples.view(np.int16).copy()).cuda()
+    sl = B.Offsets(slice_off)
+    d_out = torch.empty((n, 2), dtype=torch.int64, device="cuda")
+    d_runs = torch.zeros(sl.count * w.geometry.n_pmt + 1, dtype=torch.int32, device="cuda")
+    st = torch.zeros(1, dtype=torch.int32, device="cuda")
+    ws = {}
+
+    def go():
+        ws["p"] = B.tt_prepare_slice(d_raw, d_samples, sl, w.geometry.n_pmt, d_out, d_runs, st, ws.get("p"))
+
+    ms = _cuda_time(go, 5)
+    assert B.hits_to_host(d_out).tobytes() == np.ascontiguousarray(w.hits).tobytes(), "prepare differs from the generator"
+    byt = raw.nbytes + samples.nbytes + 16 * n
+    return {"workload": w.name + " x 0.1", "raw_hits": n, "raw_bytes_per_hit": (raw.nbytes + samples.nbytes) / n,
+            "ms": ms, "hits_per_s": n / (ms * 1e-3), "alg_bytes": byt, "frac": byt / (ms * 1e-3) / 1e9 / peak,
+            "paper": "200-300 ms of CPU time per second of data, transfer included (PAPER.md:71)"}
+
+
+class Run:
+    """One workload on the device with its buffers; step() = one pass of the whole hot path."""
+
+    def __init__(self, B, cfg, rank, scale, fused):
+        import torch
+
+        self.B, self.fused = B, fused
+        self.w = w = make_workload(cfg, rank, scale)
+        self.n = n = w.n
+        g = w.geometry
+        self.geo = B.Geometry(g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks)
+        p = w.params
+        self.prm = B.make_params(p.q_thresh, p.lc_window_ps, p.l2_window_ps, p.l2_multiplicity, p.l2_mode, p.event_half_ps)
+        self.seg, self.runs = B.Offsets(w.seg_offsets), B.Offsets(w.run_offsets)
+        self.d_in = B.hits_to_device(w.hits)
+        self.d_out = torch.empty_like(self.d_in)
+        self.seed_cap = self.event_cap = max(n // 4, 1024)
+        self.d_flags = torch.zeros(n, dtype=torch.uint8, device="cuda")
+        self.d_seeds = torch.zeros(self.seed_cap, dtype=torch.int32, device="cuda")
+        self.d_ev = torch.zeros((self.event_cap, 4), dtype=torch.int64, device="cuda")
+        self.d_cnt = torch.zeros(4, dtype=torch.int32, device="cuda")  # n_seeds, n_events, status, spare
+        self.ws = {}
+
+    def step(self):
+        B, ws, c = self.B, self.ws, self.d_cnt
+        d_ns, d_ne, d_st = c[0:1], c[1:2], c[2:3]
+        c.zero_()
+        if self.fused:
+            ws["f"] = B.tt_sort_trigger_slice(self.d_in, self.d_out, None, self.seg, self.runs, self.geo, self.prm,
+                                              self.d_flags, self.d_seeds, d_ns, d_st, ws.get("f"))
+        else:
+            ws["s"] = B.tt_sort_slice(self.d_in, self.d_out, None, self.seg, self.runs, d_st, ws.get("s"))
+            ws["t"] = B.tt_trigger_slice(self.d_out, self.seg, self.geo, self.prm, self.d_flags, self.d_seeds, d_ns, d_st,
+                                         ws.get("t"))
+        ws["e"] = B.tt_extract_events(self.d_out, self.seg, self.d_seeds, d_ns, self.prm, self.d_ev, d_ne, self.d_flags,
+                                      None, None, d_st, ws.get("e"))
+
+    def counts(self):
+        c = self.d_cnt.cpu().numpy().view(np.uint32)
+        return int(c[0]), int(c[1]), int(c[2])
+
+
+def timed_steps(B, run, steps, warmup, graph_mode, barrier, sampler=None):
+    """W warm-up steps, then exactly `steps` timed steps (CUDA events on the launching stream) -- replayed as a CUDA
+    graph when it can be captured -- then a separate profiled pass of direct launches for the per-stage times."""
+    import torch
+
+    for _ in range(max(warmup, 3)):
+        run.step()
+    barrier()
+    n_seeds, n_events, status = run.counts()
+    graph, graph_note, launches_per_replay = None, None, 0
+    if graph_mode in ("on", "auto"):
+        try:
+            cg = torch.cuda.CUDAGraph()
+            lc = B.launch_count()
+            with torch.cuda.graph(cg):
+                run.step()
+            launches_per_replay = B.launch_count() - lc
+            cg.replay()
+            torch.cuda.synchronize()
+            assert run.counts() == (n_seeds, n_events, status), "graph replay differs"
+            graph = cg
+        except Exception as ex:  # capture not possible here: time the direct launches
+            graph, graph_note = None, f"capture failed: {type(ex).__name__}"
+            torch.cuda.synchronize()
+    go = graph.replay if graph is not None else run.step
+    if graph is None:
+        B.prof_enable(True)
+    l0 = B.launch_count()
+    barrier()
+    if sampler is not None:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        go()
+    e1.record()
+    barrier()
+    clocks = sampler.stop() if sampler is not None else None
+    launches = B.launch_count() - l0 if graph is None else launches_per_replay * steps
+    ms_total = e0.elapsed_time(e1)
+    if graph is not None:  # stage breakdown from direct launches, outside the timed region
+        B.prof_enable(True)
+        run.step()         # first profiled step creates the event pool and the pinned counter buffers: not measured
+        barrier()
+        B.prof_enable(True)  # clears the marks
+        for _ in range(steps):
+            run.step()
+        barrier()
+    stages = B.prof_read()
+    B.prof_enable(False)
+    counters = {k[4:]: v[0] / max(v[1], 1) for k, v in stages.items() if k.startswith("ctr.")}
+    stages = {k: v for k, v in stages.items() if not k.startswith("ctr.")}
+    per_stage = {k: v[0] / steps for k, v in stages.items()}  # ms per step
+    per_launches = {k: v[1] / steps for k, v in stages.items()}
+    return dict(ms_step=ms_total / steps, per_stage=per_stage, per_launches=per_launches, counters=counters,
+                launches=int(launches), clocks=clocks, graph=graph is not None, graph_note=graph_note,
+                n_seeds=n_seeds, n_events=n_events, status=status)
+
+
+def stage_fracs(per_stage, n, peak):
+    """Stage-level roofline fractions: the stage's algorithmic bytes ONCE (sort 32 B/hit whatever the
+    number of merge levels, trigger 18 B/hit, events ~2 B/hit) over the summed time of all its kernels."""
+    out = {}
+    for fam, byt in ALG_BYTES.items():
+        ms = sum(v for k, v in per_stage.items() if k.split(".")[0] == fam)
+        if ms > 0:
+            out[fam] = {"alg_bytes_per_hit": byt, "ms": ms, "achieved": byt * n / (ms * 1e-3) / 1e9,
+                        "frac": byt * n / (ms * 1e-3) / 1e9 / peak}
+    return out
+
+
 def run_ours(args):
     import torch
 
@@ -208,31 +428,10 @@ def run_ours(args):
 
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     B.load()
-    w = make_workload(args.config, rank, args.scale)
-    n = w.n
-    g = w.geometry
-    geo = B.Geometry(g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks)
-    p = w.params
-    prm = B.make_params(p.q_thresh, p.lc_window_ps, p.l2_window_ps, p.l2_multiplicity, p.l2_mode, p.event_half_ps)
-    seg, runs = B.Offsets(w.seg_offsets), B.Offsets(w.run_offsets)
-    d_in = B.hits_to_device(w.hits)
-    d_out = torch.empty_like(d_in)
-    seed_cap = event_cap = max(n // 4, 1024)
-    d_flags = torch.zeros(n, dtype=torch.uint8, device="cuda")
-    d_seeds = torch.zeros(seed_cap, dtype=torch.int32, device="cuda")
-    d_ev = torch.zeros((event_cap, 4), dtype=torch.int64, device="cuda")
-    d_cnt = torch.zeros(4, dtype=torch.int32, device="cuda")  # n_seeds, n_events, status, spare
-    d_ns, d_ne, d_st = d_cnt[0:1], d_cnt[1:2], d_cnt[2:3]
-    ws = {}
-
-    def step():
-        d_cnt.zero_()
-        if args.fused == "on":
-            ws["f"] = B.tt_sort_trigger_slice(d_in, d_out, None, seg, runs, geo, prm, d_flags, d_seeds, d_ns, d_st, ws.get("f"))
-        else:
-            ws["s"] = B.tt_sort_slice(d_in, d_out, None, seg, runs, d_st, ws.get("s"))
-            ws["t"] = B.tt_trigger_slice(d_out, seg, geo, prm, d_flags, d_seeds, d_ns, d_st, ws.get("t"))
-        ws["e"] = B.tt_extract_events(d_out, seg, d_seeds, d_ns, prm, d_ev, d_ne, d_flags, None, None, d_st, ws.get("e"))
+    fused = args.fused == "on"
+    run = Run(B, args.config, rank, args.scale, fused)
+    w, n, geo, prm, seg, runs = run.w, run.n, run.geo, run.prm, run.seg, run.runs
+    d_out, seed_cap, event_cap = run.d_out, run.seed_cap, run.event_cap
 
     def barrier():
         torch.cuda.synchronize()
@@ -240,93 +439,48 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(max(args.warmup, 3)):
-        step()
-    barrier()
-    counts = d_cnt.cpu().numpy().view(np.uint32)
-    n_seeds, n_events, status = int(counts[0]), int(counts[1]), int(counts[2])
-    l1_frac = float((d_flags & 4).ne(0).float().mean().item())
-    inevt_frac = float((d_flags & 32).ne(0).float().mean().item())
-
-    # The step (24 launches + 3 memsets) is captured once in a CUDA graph and replayed in the timed region: the library
-    # allocates nothing and never synchronises in its hot calls.  Launch gaps are most of cfg0 / cfg1 (0.22 -> 0.09 ms,
-    # 0.24 -> 0.11 ms) and still ~0.1 ms of the large configs.  The per-stage events cannot be recorded inside a replay:
-    # they come from a separate, untimed, profiled pass of direct launches.
-    use_graph = args.graph in ("on", "auto")
-    graph, graph_note, launches_per_replay = None, None, 0
-    if use_graph:
-        try:
-            cg = torch.cuda.CUDAGraph()
-            lc = B.launch_count()
-            with torch.cuda.graph(cg):
-                step()
-            launches_per_replay = B.launch_count() - lc
-            cg.replay()
-            torch.cuda.synchronize()
-            chk = d_cnt.cpu().numpy().view(np.uint32)
-            assert (int(chk[0]), int(chk[1]), int(chk[2])) == (n_seeds, n_events, status), "graph replay differs"
-            graph = cg
-        except Exception as ex:  # capture not possible here: time the direct launches
-            graph, graph_note = None, f"capture failed: {type(ex).__name__}"
-            torch.cuda.synchronize()
-    run = graph.replay if graph is not None else step
-
     sampler = ClockSampler(local)
-    if graph is None:
-        B.prof_enable(True)
-    l0 = B.launch_count()
-    barrier()
-    sampler.start()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for _ in range(args.steps):
-        run()
-    e1.record()
-    barrier()
-    clocks = sampler.stop()
-    launches = B.launch_count() - l0 if graph is None else launches_per_replay * args.steps
-    ms_total = e0.elapsed_time(e1)
-    if graph is not None:  # stage breakdown from direct launches, outside the timed region
-        B.prof_enable(True)
-        step()             # first profiled step creates the event pool and the pinned counter buffers: not measured
-        barrier()
-        B.prof_enable(True)  # clears the marks
-        for _ in range(args.steps):
-            step()
-        barrier()
-    stages = B.prof_read()
-    B.prof_enable(False)
-    ms_step = ms_total / args.steps
+    m = timed_steps(B, run, args.steps, args.warmup, args.graph, barrier, sampler)
+    n_seeds, n_events, status = m["n_seeds"], m["n_events"], m["status"]
+    l1_frac = float((run.d_flags & 4).ne(0).float().mean().item())
+    inevt_frac = float((run.d_flags & 32).ne(0).float().mean().item())
+    clocks, launches, per_stage, counters = m["clocks"], m["launches"], m["per_stage"], m["counters"]
+    ms_step_local = m["ms_step"]
     from paper_1411_3968_b200 import sharding
 
-    ms_step, n_total = sharding.reduce_timing(ms_step, n, "cuda")  # max over ranks, whole-job hits
+    ms_step, n_total = sharding.reduce_timing(ms_step_local, n, "cuda")  # max over ranks, whole-job hits
     value = n_total / (ms_step * 1e-3)
 
-    # ---- roofline of the dominant kernel (device time from the stage events of the timed steps) ----
+    # ---- roofline of the dominant kernel (device time from the stage events of the profiled steps) ----
     peak, peak_src = peaks()
-    counters = {k[4:]: v[0] / max(v[1], 1) for k, v in stages.items() if k.startswith("ctr.")}
-    stages = {k: v for k, v in stages.items() if not k.startswith("ctr.")}
-    per_stage = {k: v[0] / args.steps for k, v in stages.items()}  # ms per step
     dom = max(per_stage, key=per_stage.get) if per_stage else None
     roof = None
     if dom:
-        launches_dom = stages[dom][1] / args.steps
-        alg = ALG_BYTES[dom.split(".")[0]] * n  # bytes the whole stage family must move once per step
-        # a stage that runs several times per step (radix passes) still has to move the algorithmic bytes once
+        launches_dom = m["per_launches"][dom]
+        fam = dom.split(".")[0]
+        # one launch of a merge-level tile kernel moves every hit once: 16 B read + 16 B written (+ 1 flag byte when L1
+        # is fused into it).  NOTE: with two merge levels EACH level is credited these bytes here; the stage-level
+        # figure below (`stage_frac`) counts the sort's 32 B/hit once, whatever the number of levels.
+        alg = ALG_BYTES[fam] * n
         dur_ms = per_stage[dom]
         ach = alg / (dur_ms * 1e-3) / 1e9
-        traffic = None  # dram__bytes_read + write per launch from the committed ncu --set full summary
+        traffic = None  # dram__bytes_read + write per launch from the committed ncu --set full summary of THIS build
         tp = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tp):
             for ln in open(tp).read().splitlines()[1:]:
                 f = ln.split(",")
                 if len(f) >= 3 and f[0] == f"cfg{args.config}" and f[1] == dom:
                     traffic = float(f[2])
+        sf = stage_fracs(per_stage, n, peak)
         roof = {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": traffic, "peak_source": peak_src, "alg_bytes_per_launch": alg / max(launches_dom, 1),
-                "launches_per_step": launches_dom, "kernel_ms_per_step": dur_ms,
-                "share_of_step": dur_ms / (ms_total / args.steps)}
-    pipe_ach = ALG_BYTES_PIPELINE * n / (ms_total / args.steps * 1e-3) / 1e9  # this rank
+                "traffic": traffic, "traffic_source": "profiles/traffic.csv: ncu --set full capture of this build (not "
+                "measured inside this run; ncu cannot run in the timed process)", "peak_source": peak_src,
+                "alg_bytes_per_launch": alg / max(launches_dom, 1), "launches_per_step": launches_dom,
+                "kernel_ms_per_step": dur_ms, "share_of_step": dur_ms / ms_step_local,
+                "stage_note": "with --fused on the L1 step runs INSIDE the last sort.merge_tile kernel, so its time is "
+                              "in the sort family and the trig family holds the edge pass, compaction, L2 and seeds",
+                "stage_frac": sf.get(fam, {}).get("frac"), "stages": sf}
+    pipe_ach = ALG_BYTES_PIPELINE * n / (ms_step_local * 1e-3) / 1e9  # this rank
 
     # ---- level-0 N-in-TW trigger (tt_l0_ntw) on the sorted hits of this workload: timed on its
     # own, NOT part of the step above.  N7TW1000 for the 32-PMT tower, N7TW500 otherwise.
@@ -405,34 +559,94 @@ def run_ours(args):
         h_cnt = np.zeros(4, dtype=np.uint32)
         vp = ctypes.c_void_p
 
-        def host_step():
-            rc = L.tt_process_host(ctx, vp(h_in.data_ptr()), vp(0), vp(h_flags.data_ptr()), ctypes.c_uint32(n),
-                                   seg.h.ctypes.data_as(vp), ctypes.c_uint32(seg.count), runs.h.ctypes.data_as(vp),
-                                   ctypes.c_uint32(runs.count), geo.handle, ctypes.byref(prm), vp(h_seeds.data_ptr()),
-                                   vp(h_ev.data_ptr()), h_cnt.ctypes.data_as(vp))
+        def host_args(cnt):
+            return (ctx, vp(h_in.data_ptr()), vp(0), vp(h_flags.data_ptr()), ctypes.c_uint32(n),
+                    seg.h.ctypes.data_as(vp), ctypes.c_uint32(seg.count), runs.h.ctypes.data_as(vp),
+                    ctypes.c_uint32(runs.count), geo.handle, ctypes.byref(prm), vp(h_seeds.data_ptr()),
+                    vp(h_ev.data_ptr()), cnt.ctypes.data_as(vp))
+
+        def host_step():  # the synchronous call: upload, compute, read back, return
+            rc = L.tt_process_host(*host_args(h_cnt))
             if rc != 0:
                 raise SystemExit(f"tt_process_host failed: {rc}")
 
         host_step()
         barrier()
-        k2 = max(1, min(args.steps, 5))
+        k2 = max(2, min(args.steps, 6))
         t0 = time.perf_counter()
         for _ in range(k2):
             host_step()
+        dt_sync = (time.perf_counter() - t0) / k2
+        assert int(h_cnt[0]) == n_seeds and int(h_cnt[1]) == n_events, "host path disagrees with device path"
+        # successive slices back to back: tt_host_submit / tt_host_wait, two slices in flight -- the upload
+        # of slice k + 1 overlaps the compute of slice k and the read-back of slice k - 1.  Every slice is uploaded,
+        # computed and read back inside the timed region; the time is per slice at steady state.
+        cnts = [np.zeros(4, dtype=np.uint32) for _ in range(2)]
+        barrier()
+        t0 = time.perf_counter()
+        for k in range(k2):
+            rc = L.tt_host_submit(*host_args(cnts[k & 1]))
+            if rc != 0:
+                raise SystemExit(f"tt_host_submit failed: {rc}")
+            if k >= 1 and L.tt_host_wait(ctx) != 0:
+                raise SystemExit("tt_host_wait failed")
+        if L.tt_host_wait(ctx) != 0:
+            raise SystemExit("tt_host_wait failed")
         dt = (time.perf_counter() - t0) / k2
+        for c2 in cnts:
+            assert int(c2[0]) == n_seeds and int(c2[1]) == n_events, "pipelined host path disagrees with device path"
         dt, _ = sharding.reduce_timing(dt, n, "cuda")
         ns, ne = int(min(h_cnt[0], seed_cap)), int(min(h_cnt[1], event_cap))
+        h2d = int(16 * n + 4 * (seg.count + 1) + 4 * (runs.count + 1))
+        d2h = int(n + 4 * ns + 32 * ne + 12)
+        # PCIe floor of one slice: its upload at the H2D rate measured right here on a plain pinned copy of the same size
+        d_tmp = torch.empty_like(run.d_in)
+        d_tmp.copy_(h_in, non_blocking=True)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        d_tmp.copy_(h_in, non_blocking=True)
+        torch.cuda.synchronize()
+        floor_ms = 1e3 * (time.perf_counter() - t0)
+        del d_tmp
         e2e = {"value": n_total / dt, "unit": "hits/s", "ms_per_step": 1e3 * dt,
-               "h2d_bytes_per_step": int(16 * n + 4 * (seg.count + 1) + 4 * (runs.count + 1)),
-               "d2h_bytes_per_step": int(n + 4 * ns + 32 * ne + 12),
-               "api": "tt_process_host (pinned host buffers; returns flags, seeds, events)"}
-        assert int(h_cnt[0]) == n_seeds and int(h_cnt[1]) == n_events, "host path disagrees with device path"
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "pcie_floor_ms": floor_ms, "vs_pcie_floor": 1e3 * dt / floor_ms,
+               "ms_per_step_synchronous_call": 1e3 * dt_sync,
+               "api": "tt_host_submit / tt_host_wait, two slices in flight (pinned host buffers; every slice uploaded, "
+                      "computed, flags + seeds + events read back); ms_per_step_synchronous_call = tt_process_host"}
         L.tt_host_ctx_destroy(ctx)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         on, odt, sample, _ = time_oracle(args.config)
         cpu = {"value": on / odt, "unit": "hits/s", "cores": 1, "kind": "oracle", "sample": sample}
+        try:
+            cpu["all_cores"] = time_oracle_all_cores(args.config)
+        except Exception as ex:  # the reported baseline must not take the bench line down
+            cpu["all_cores"] = {"error": type(ex).__name__}
+
+    # ---- the other configs (short runs; the driver's record then covers all five), the unsorted-input radix path and
+    # the preparation step (tt_prepare_slice), each timed on its own, none part of the step above
+    extra = None
+    if rank == 0 and world == 1 and not args.no_extra:
+        extra = {"configs": {}}
+        del run
+        torch.cuda.empty_cache()
+        for c2 in [c for c in (0, 1, 2, 3, 4) if c != args.config]:
+            r2 = Run(B, c2, 0, 1.0, fused)
+            m2 = timed_steps(B, r2, max(3, min(args.steps, 10)), 3, args.graph, barrier)
+            extra["configs"][f"cfg{c2}"] = {
+                "workload": r2.w.name, "hits": r2.n, "ms_per_step": m2["ms_step"],
+                "ms_per_200ms_slice": m2["ms_step"] / r2.w.n_slices, "hits_per_s": r2.n / (m2["ms_step"] * 1e-3),
+                "pipeline_frac": ALG_BYTES_PIPELINE * r2.n / (m2["ms_step"] * 1e-3) / 1e9 / peak,
+                "stages": {k: v["frac"] for k, v in stage_fracs(m2["per_stage"], r2.n, peak).items()},
+                "n_seeds": m2["n_seeds"], "n_events": m2["n_events"], "status": m2["status"]}
+            if c2 == 1:
+                extra["radix_unsorted_input"] = time_radix(B, r2, peak)
+            if c2 == 2:
+                extra["prepare"] = time_prepare(B, peak)
+            del r2
+            torch.cuda.empty_cache()
 
     if rank == 0:
         slices = w.n_slices
@@ -441,11 +655,15 @@ def run_ours(args):
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "int64", "data": "synthetic",
             "config": {"workload": w.name, "hits_per_rank": n, "slices_per_step": slices,
+                       "timed_step": ("tt_sort_trigger_slice (sort + L1 fused + L2 + seeds)" if fused else
+                                      "tt_sort_slice + tt_trigger_slice") + " + tt_extract_events with INEVT tagging "
+                                     "(SURVEY.md 8(d) times the events separately: they are INSIDE this step, "
+                                     "ev.* in stages_ms_per_step)",
                        "ms_per_200ms_slice": ms_step / slices, "l2_flush": "inputs larger than L2 (16 B x n)"
                        if 16 * n > 130e6 else "inputs fit in L2: not flushed (launch-bound config)",
                        "n_seeds": n_seeds, "n_events": n_events, "status": status, "l1_fraction": l1_frac,
                        "inevt_fraction": inevt_frac, "parallelism": f"slice-per-gpu x{world}",
-                       "cuda_graph": graph is not None, "cuda_graph_note": graph_note},
+                       "cuda_graph": m["graph"], "cuda_graph_note": m["graph_note"]},
             "clocks": clocks, "gpu_launches": int(launches),
             "roofline": roof,
             "pipeline_roofline": {"alg_bytes_per_hit": ALG_BYTES_PIPELINE, "achieved": pipe_ach, "peak": peak,
@@ -453,7 +671,7 @@ def run_ours(args):
             "stages_ms_per_step": {k: round(v, 5) for k, v in sorted(per_stage.items())},
             "counters": counters,
             "l0_ntw": l0,
-            "e2e": e2e, "cpu_baseline": cpu,
+            "e2e": e2e, "cpu_baseline": cpu, "extra": extra,
         }
         print(json.dumps(out))
     if dist is not None:
@@ -474,6 +692,7 @@ def main():
                     help="on: tt_sort_trigger_slice (L1 fused into the last merge level); off: the three separate calls")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-extra", action="store_true", help="skip the short runs of the other configs / radix / prepare")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

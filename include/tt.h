@@ -227,7 +227,7 @@ int tt_prepare_slice(const tt_raw_hit* d_raw, const uint16_t* d_samples, uint32_
  * tt_host_ctx_create allocates, once, device buffers and workspaces for slices of up to max_n hits,
  * max_seg segments and max_runs runs, and an internal stream; tt_host_ctx_destroy frees them.
  * tt_process_host copies the hits and offsets to the device (h_in pinned or pageable), runs
- * tt_sort_slice -> tt_trigger_slice -> tt_extract_events (with INEVT tagging), copies back the
+ * tt_sort_trigger_slice -> tt_extract_events (with INEVT tagging), copies back the
  * sorted hits (h_sorted nullable), the flags (h_flags nullable), the first min(n_seeds, seed_cap)
  * seeds and min(n_events, event_cap) events, and synchronises.
  * h_counts[3] = {n_seeds, n_events, status}.  h_run_offsets NULL = unsorted input. */
@@ -235,6 +235,17 @@ typedef struct tt_host_ctx tt_host_ctx;
 int tt_host_ctx_create(tt_host_ctx** c, uint32_t max_n, uint32_t max_seg, uint32_t max_runs, uint32_t seed_cap,
                        uint32_t event_cap);
 int tt_host_ctx_destroy(tt_host_ctx* c);
+/* The same, two slices deep, for slices that arrive back to back: tt_host_submit enqueues the upload of
+ * a slice, its compute and the read-back of its results on three streams and returns at once; the upload of the next
+ * slice then overlaps this slice's compute and the previous slice's read-back.  tt_host_wait blocks until the OLDEST
+ * submitted slice is complete (its h_* buffers and h_counts are then valid).  At most two slices may be in flight
+ * (a third tt_host_submit returns TT_E_INVAL); the host buffers of a slice must stay untouched until its wait returns.
+ * tt_process_host = tt_host_submit + tt_host_wait. */
+int tt_host_submit(tt_host_ctx* c, const tt_hit* h_in, tt_hit* h_sorted, uint8_t* h_flags, uint32_t n,
+                   const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* h_run_offsets, uint32_t n_runs,
+                   const tt_geometry* g, const tt_params* p, uint32_t* h_seeds, tt_event* h_events,
+                   uint32_t* h_counts);
+int tt_host_wait(tt_host_ctx* c);
 int tt_process_host(tt_host_ctx* c, const tt_hit* h_in, tt_hit* h_sorted, uint8_t* h_flags, uint32_t n,
                     const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* h_run_offsets,
                     uint32_t n_runs, const tt_geometry* g, const tt_params* p, uint32_t* h_seeds,

@@ -269,3 +269,56 @@ def test_two_host_threads_two_streams(B, oracle_lib):
     for t in th:
         t.join()
     assert not errs, errs
+
+
+def test_host_pipeline_submit_wait(B, oracle_lib):
+    """tt_host_submit / tt_host_wait with two slices in flight (different slices, alternating), against the oracle;
+    a third submit is refused; tt_process_host is refused while slices are in flight."""
+    import ctypes
+
+    ws_ = [W.make_config(1, time_scale=0.03), W.make_config(1, time_scale=0.05, seed_offset=3)]
+    os_ = [oracle_chain(w.hits, w.seg_offsets, w.geometry, w.params) for w in ws_]
+    geo = _geo(B, ws_[0].geometry)
+    prm = _prm(B, ws_[0].params)
+    L = B.load()
+    ctx = ctypes.c_void_p(0)
+    nmax = max(w.n for w in ws_)
+    assert L.tt_host_ctx_create(ctypes.byref(ctx), nmax, 4, len(ws_[0].run_offsets), nmax, nmax) == 0
+    vp = lambda a: a.ctypes.data_as(ctypes.c_void_p)
+    bufs = []
+    for w in ws_:
+        bufs.append(dict(hin=np.ascontiguousarray(w.hits), srt=np.zeros(w.n, dtype=B.HIT_DTYPE), fl=np.zeros(w.n, dtype=np.uint8),
+                         seeds=np.zeros(nmax, dtype=np.uint32), ev=np.zeros(nmax, dtype=B.EVENT_DTYPE),
+                         cnt=np.zeros(3, dtype=np.uint32), seg=np.ascontiguousarray(w.seg_offsets, dtype=np.uint32),
+                         runs=np.ascontiguousarray(w.run_offsets, dtype=np.uint32)))
+
+    def submit(k, want_sorted=True):
+        b, w = bufs[k], ws_[k]
+        return L.tt_host_submit(ctx, vp(b["hin"]), vp(b["srt"]) if want_sorted else ctypes.c_void_p(0), vp(b["fl"]),
+                                ctypes.c_uint32(w.n), vp(b["seg"]), ctypes.c_uint32(len(b["seg"]) - 1), vp(b["runs"]),
+                                ctypes.c_uint32(len(b["runs"]) - 1), geo.handle, ctypes.byref(prm), vp(b["seeds"]),
+                                vp(b["ev"]), vp(b["cnt"]))
+
+    def check(k, want_sorted=True):
+        b, o = bufs[k], os_[k]
+        if want_sorted:
+            assert b["srt"].tobytes() == o["sorted"].tobytes()
+        assert (b["fl"] == o["flags"]).all()
+        assert b["cnt"][0] == len(o["seeds"]) and (b["seeds"][: b["cnt"][0]] == o["seeds"]).all()
+        assert b["cnt"][1] == len(o["events"]) and b["ev"][: b["cnt"][1]].tobytes() == o["events"].tobytes()
+        assert b["cnt"][2] == 0
+
+    assert L.tt_host_wait(ctx) == B.TT_E_INVAL  # nothing in flight
+    for want_sorted in (True, False):
+        assert submit(0, want_sorted) == 0
+        for it in range(1, 6):
+            assert submit(it & 1, want_sorted) == 0
+            if it == 1:
+                assert submit(0, want_sorted) == B.TT_E_INVAL  # both slots busy
+            assert L.tt_host_wait(ctx) == 0
+            check((it - 1) & 1, want_sorted)
+            for key in ("srt", "fl", "seeds", "ev", "cnt"):
+                bufs[(it - 1) & 1][key][...] = 0 if key != "fl" else 0xEE
+        assert L.tt_host_wait(ctx) == 0
+        check(5 & 1, want_sorted)
+    L.tt_host_ctx_destroy(ctx)
