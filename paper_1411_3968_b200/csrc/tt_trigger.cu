@@ -398,7 +398,7 @@ constexpr int kRowHalo = kRowSpan;       // a window of <= kRowSpan hits never l
 constexpr int kRowStage = kRowTile + 2 * kRowHalo;  // staged records per tile: always [x0 - 256, x0 + 512)
 constexpr int kRowPer = kRowStage / kRowTile;  // 3
 constexpr int kRowWords = 10;            // (31 + kRowSpan) / 32 + 1 = 9, padded to a 48-byte row
-constexpr int kPairList = 2 * 256 * 16;   // pair list of one round: 256 hits x 16 offsets x (later + before-tile) candidates
+constexpr int kPairList = 256 * 16;       // pair lists of one round: 8 warps x (32 hits x 16 offsets)
 constexpr int kPairBytesMax = 16384;     // tower-pair byte table in shared memory: n_tower <= 128
 constexpr uint32_t kWide = 0xFFFFFFFFu;
 
@@ -518,36 +518,17 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
         const uint32_t prow = (tpx >> 16) * nt;
         const bool emits = x < x1 && any_edge && tpx != kBadTp && (nt > 1 || blk_single >= 0);
         const uint32_t fwd_end = emits ? (wide ? min(hi, t1l) : hi) : 0u;   // later candidates: [xl + 1, fwd_end)
-        const uint32_t back_end = (emits && !wide) ? min(xl, t0l) : 0u;      // candidates before the tile: [lo, back_end)
-        const uint32_t reach = max(fwd_end > xl + 1u ? fwd_end - xl - 1u : 0u, back_end > lo ? back_end - lo : 0u);
-        const uint32_t lane = tid & 31u;
-        // Every warp keeps its own pair list (32 hits x 16 offsets x 2 streams = 1024 entries) and tests its own pairs:
-        // the rounds need no block-wide barrier and no shared counter (the row bits are OR-ed with atomics anyway), so
-        // a warp with a short reach does not wait for the dense ones round by round.
-        uint16_t* const wlist = sm.list + (tid >> 5) * (uint32_t)(kPairList / (kRowTile / 32));
-        for (uint32_t r = 0;; ++r) {
-            if (!__any_sync(0xffffffffu, reach > 16u * r)) break;
-            uint32_t np = 0;  // warp-uniform
-            // one stream at a time: the candidates before the tile exist for the first hits of the tile only
-            // (most warps leave that loop at its first vote)
-#pragma unroll 1
-            for (uint32_t stream = 0; stream < 2u; ++stream) {
-                const uint32_t y0 = (stream ? lo : xl + 1u) + 16u * r, yend = stream ? back_end : fwd_end;
-                for (uint32_t dd = 0; dd < 16u; ++dd) {
-                    const uint32_t y = y0 + dd;
-                    bool c = y < yend;
-                    if (!__any_sync(0xffffffffu, c)) break;  // offsets only grow
-                    if (c) {
-                        const uint32_t tpy = sm.tp[y];
-                        c = tpy != kBadTp && !(pair_smem && s_pair[prow + (tpy >> 16)] == 0xFF);
-                    }
-                    const uint32_t mk = __ballot_sync(0xffffffffu, c);
-                    if (c) wlist[np + (uint32_t)__popc(mk & ((1u << lane) - 1u))] = (uint16_t)((stream << 12) | (tid << 4) | dd);
-                    np += (uint32_t)__popc(mk);
-                }
-            }
-            __syncwarp();
-            for (uint32_t p0 = lane; p0 < np; p0 += 4u * 32u) {  // four pairs per thread in flight: the table gather is the latency
+        const uint32_t reach = fwd_end > xl + 1u ? fwd_end - xl - 1u : 0u;
+        const uint32_t lane = tid & 31u, warp = tid >> 5;
+        // Every warp keeps its own pair list and tests its own pairs: the rounds need no block-wide barrier and no
+        // shared counter (the row bits are OR-ed with atomics anyway), so a warp with a short reach does not wait for
+        // the dense ones round by round.
+        uint16_t* const wlist = sm.list + warp * (uint32_t)(kPairList / (kRowTile / 32));
+        // the listed pairs, one thread per pair, four in flight (the table gather is the latency).  mode 0: entry =
+        // tile index of x << 4 | offset, y = x + 1 + base + offset; mode 1: entry = tile index << 3 | offset,
+        // y = lo(x) + base + offset
+        auto test_pairs = [&](uint32_t np, uint32_t mode, uint32_t base) {
+            for (uint32_t p0 = lane; p0 < np; p0 += 4u * 32u) {
                 uint32_t xt4[4], y4[4];
                 int32_t lim4[4];
 #pragma unroll
@@ -556,8 +537,8 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
                     lim4[u] = -1; xt4[u] = 0; y4[u] = 0;
                     if (p < np) {
                         const uint32_t pr = wlist[p];
-                        const uint32_t xt = (pr >> 4) & 0xFFu, xs = t0l + xt;  // tile index / staged index of x
-                        const uint32_t y = ((pr & 0x1000u) ? sm.lo[xt] : xs + 1u) + 16u * r + (pr & 15u);  // staged index of y
+                        const uint32_t xt = mode ? pr >> 3 : pr >> 4, xs = t0l + xt;  // tile index / staged index of x
+                        const uint32_t y = (mode ? sm.lo[xt] + (pr & 7u) : xs + 1u + (pr & 15u)) + base;  // staged index of y
                         const uint32_t tpa = sm.tp[xs], tpb = sm.tp[y];
                         int32_t bi;
                         if (nt == 1) bi = blk_single;
@@ -588,7 +569,67 @@ __global__ void __launch_bounds__(kRowTile) l2_rows_kernel(const L1Rec* __restri
                     }
                 }
             }
+        };
+        // ---- phase A: every warp walks its own 32 hits in lockstep over the LATER candidates y = x + 1 + d, 16
+        // offsets per round (a pair inside the tile is owned by its earlier hit, so it is tested once)
+        for (uint32_t r = 0;; ++r) {
+            if (!__any_sync(0xffffffffu, reach > 16u * r)) break;
+            uint32_t np = 0;  // warp-uniform
+            const uint32_t y0 = xl + 1u + 16u * r;
+            // the 16 offsets of the round in three straight-line sweeps (16 independent loads each, no early exit)
+            uint32_t tp16[16];
+#pragma unroll
+            for (uint32_t dd = 0; dd < 16u; ++dd) tp16[dd] = y0 + dd < fwd_end ? sm.tp[y0 + dd] : kBadTp;
+            uint32_t cm = 0;  // bit dd: candidate on a connected tower
+#pragma unroll
+            for (uint32_t dd = 0; dd < 16u; ++dd) {
+                bool c = tp16[dd] != kBadTp;
+                if (c && pair_smem) c = s_pair[prow + (tp16[dd] >> 16)] != 0xFF;
+                cm |= (c ? 1u : 0u) << dd;
+            }
+#pragma unroll
+            for (uint32_t dd = 0; dd < 16u; ++dd) {
+                const bool c = (cm >> dd) & 1u;
+                const uint32_t mk = __ballot_sync(0xffffffffu, c);
+                if (c) wlist[np + (uint32_t)__popc(mk & ((1u << lane) - 1u))] = (uint16_t)((tid << 4) | dd);
+                np += (uint32_t)__popc(mk);
+            }
+            __syncwarp();
+            test_pairs(np, 0u, 16u * r);
             __syncwarp();  // the list is rewritten in the next round
+        }
+        // ---- phase B: the candidates BEFORE the tile, y = lo(x) + d < first hit of the tile.  Only the first hits of
+        // a tile have them (the whole load of an extra pass for the first warp, and the rest of the block waited for
+        // it at the barrier below): now shared by all warps -- batch by batch of 32 hits, warp w takes the offsets
+        // d with (d / 8) % 8 == w.
+        for (uint32_t bq = 0; bq < (uint32_t)kRowTile / 32u; ++bq) {
+            const uint32_t xt = 32u * bq + lane;
+            uint32_t lo_b = 0, cnt_b = 0, prow_b = 0;
+            if (x0 + xt < x1) {
+                const uint32_t l0 = sm.lo[xt], tpb = sm.tp[t0l + xt];
+                if (l0 != kWide && l0 < t0l && any_edge && tpb != kBadTp && (nt > 1 || blk_single >= 0)) {
+                    lo_b = l0; cnt_b = t0l - l0; prow_b = (tpb >> 16) * nt;
+                }
+            }
+            if (!__any_sync(0xffffffffu, cnt_b > 0u)) break;  // windows move forward: no later batch has any either
+            for (uint32_t base = 8u * warp;; base += 8u * (uint32_t)(kRowTile / 32)) {
+                if (!__any_sync(0xffffffffu, cnt_b > base)) break;
+                uint32_t np = 0;
+#pragma unroll
+                for (uint32_t dd = 0; dd < 8u; ++dd) {
+                    bool c = base + dd < cnt_b;
+                    if (c) {
+                        const uint32_t tpy = sm.tp[lo_b + base + dd];
+                        c = tpy != kBadTp && !(pair_smem && s_pair[prow_b + (tpy >> 16)] == 0xFF);
+                    }
+                    const uint32_t mk = __ballot_sync(0xffffffffu, c);
+                    if (c) wlist[np + (uint32_t)__popc(mk & ((1u << lane) - 1u))] = (uint16_t)((xt << 3) | dd);
+                    np += (uint32_t)__popc(mk);
+                }
+                __syncwarp();
+                test_pairs(np, 1u, base);
+                __syncwarp();
+            }
         }
         __syncthreads();  // all rows complete (bits come from other warps too)
         // ---- rows out -------------------------------------------------------------------------------------
@@ -1081,7 +1122,7 @@ static int trigger_run(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg
     const uint32_t nt2 = g->dev.n_tower * g->dev.n_tower;
     const uint32_t pair_smem = (g->dev.n_tower > 1 && nt2 <= (uint32_t)kPairBytesMax && g->dev.n_blocks <= 255u) ? 1u : 0u;
     const size_t rows_smem = sizeof(RowSmem) + (pair_smem ? ((nt2 + 15u) & ~15u) : 0);
-    TT_K(l2_rows_kernel)<<<sms * 4, kRowTile, rows_smem, s>>>(
+    TT_K(l2_rows_kernel)<<<sms * 5, kRowTile, rows_smem, s>>>(
         plan.l1, plan.m_total, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps, p->l2_multiplicity, p->l2_mode,
         pair_smem, d_flags, plan.l2bit, plan.rows, plan.slow_list, plan.slow_cnt);
     prof_mark(s, "trig.l2_clique");
