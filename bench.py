@@ -488,6 +488,7 @@ def run_ours(args):
     l0 = None
     if rank == 0:
         l0_n, l0_tw = 7, (1_000_000 if args.config == 0 else 500_000)
+        g_multi = w.geometry.n_tower > 1
         d_l0 = torch.empty(n, dtype=torch.uint8, device="cuda")
         d_l0n = torch.zeros(1, dtype=torch.int32, device="cuda")
         for _ in range(3):
@@ -503,7 +504,12 @@ def run_ours(args):
         l0_ach = 17.0 * n / (l0_ms * 1e-3) / 1e9
         l0 = {"kernel": "l0_ntw_kernel", "multiplicity": l0_n, "window_ps": l0_tw, "ms": l0_ms,
               "hits_per_s": n / (l0_ms * 1e-3), "alg_bytes_per_hit": 17, "achieved": l0_ach, "peak": peak,
-              "unit": "GB/s", "frac": l0_ach / peak, "n_start": int(d_l0n.cpu().numpy().view(np.uint32)[0])}
+              "unit": "GB/s", "frac": l0_ach / peak, "n_start": int(d_l0n.cpu().numpy().view(np.uint32)[0]),
+              "note": ("level-0 / DN / pair / combine legs: separate calls on the sorted hits, outside the timed step.  "
+                       "The paper applies N7TW500, SC, FC and AFC per 84-PMT tower; on the multi-tower stream of "
+                       "cfg4 (100 towers superimposed, 462 hits/us) every window start fires, so these cfg4 "
+                       "figures are BANDWIDTH PROBES of the kernels, not trigger results") if g_multi else
+                      "separate calls on the sorted hits, outside the timed step"}
         # the paper's pair seeds (SC / FC / AFC) and its combination with the level-0 windows
         # (PAPER.md:65, 73): tt_pair_seeds 16 B read + 1 B written per hit, tt_l0_combine 2 B read + 1 B written
         gw = w.geometry

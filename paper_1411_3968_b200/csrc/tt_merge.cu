@@ -69,7 +69,11 @@ __global__ void __launch_bounds__(1024) merge_groups_kernel(LevelDev lv, const u
 
 // ---- plan step 2: per group: hit count, tile count, key range, tile width; prefixes.  One block,
 // one warp per group (lanes over the group's runs).
-__global__ void __launch_bounds__(1024) merge_setup_kernel(LevelDev lv, const uint4* __restrict__ hits, uint32_t n) {
+// run_kmin / run_kmax (nullable): the key range of every run when the runs are the previous level's groups whose hits
+// are not written yet (the previous level's tile kernel emits this level's splits, see emit_next_splits)
+__global__ void __launch_bounds__(1024) merge_setup_kernel(LevelDev lv, const uint4* __restrict__ hits, uint32_t n,
+                                                           const uint64_t* __restrict__ run_kmin,
+                                                           const uint64_t* __restrict__ run_kmax) {
     __shared__ uint32_t sm[33];
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     // pass A: per-group ranges (warp per group)
@@ -78,8 +82,9 @@ __global__ void __launch_bounds__(1024) merge_setup_kernel(LevelDev lv, const ui
         uint64_t kmin = ~0ull, kmax = 0;
         for (uint32_t r = r0 + lane; r < r1; r += 32) {
             const uint32_t a = lv.roff[r], b = lv.roff[r + 1];
+            lv.run_group[r] = g;
             if (b > a) {
-                const uint64_t k0 = key_at(hits, a), k1 = key_at(hits, b - 1);
+                const uint64_t k0 = run_kmin ? run_kmin[r] : key_at(hits, a), k1 = run_kmax ? run_kmax[r] : key_at(hits, b - 1);
                 kmin = k0 < kmin ? k0 : kmin;
                 kmax = k1 > kmax ? k1 : kmax;
             }
@@ -94,6 +99,7 @@ __global__ void __launch_bounds__(1024) merge_setup_kernel(LevelDev lv, const ui
             const uint32_t n_g = lv.roff[r1] - lv.roff[r0];
             const uint32_t nt = tiles_for(n_g);
             lv.gT0[g] = kmin;
+            lv.gKmax[g] = kmax;
             uint64_t dt = nt ? (kmax >= kmin ? (kmax - kmin) / nt + 1 : 1) : 1;
             if (dt == 0) dt = ~0ull;  // one tile over the whole key range, 2^64 - 1: the + 1 wrapped
             lv.gDT[g] = dt;
@@ -234,6 +240,90 @@ __global__ void __launch_bounds__(256, 8) merge_partition_kernel(LevelDev lv, co
     if (j == 0 && k < nt) {
         lv.tile_desc[lv.tbase[g] + k] = make_uint4(g, r0, K, k);
         lv.tile_desc2[lv.tbase[g] + k] = make_uint2(lv.sbase[g] + k * K, lv.tbase[g] + g + k);
+    }
+}
+
+// ---- the next level's split table without a partition pass -----------------------------------------------
+// A merge level's tile kernel has every sorted tile in shared memory (or has just written it), and the next level's
+// runs ARE this level's groups: the position of a next-level boundary T1 inside run j1 is the tile's output base plus a
+// lower bound inside the one tile whose key range holds T1.  So the tile kernels of level l write level l + 1's
+// split rows and tile-base sums themselves (a few dozen binary searches in shared memory per tile) and the
+// partition kernel -- 0.16 ms and 0.6 GB of DRAM probes on the 100-tower config -- runs for level 0 only.
+// merge_init_next_kernel writes what no tile writes: row 0 (run starts), the rows of empty runs, the tile descriptors.
+__global__ void __launch_bounds__(256, 8) merge_init_next_kernel(LevelDev lv, uint32_t total) {
+    const uint32_t id = blockIdx.x * blockDim.x + threadIdx.x;
+    if (id >= total) return;
+    uint32_t lo = 0, hi = lv.G;  // group with sbase[g] <= id < sbase[g+1]
+    while (hi - lo > 1) { const uint32_t mid = (lo + hi) >> 1; if (lv.sbase[mid] <= id) lo = mid; else hi = mid; }
+    const uint32_t g = lo;
+    const uint32_t r0 = lv.gfirst[g], K = lv.gfirst[g + 1] - r0;
+    const uint32_t local = id - lv.sbase[g];
+    const uint32_t nt = lv.tbase[g + 1] - lv.tbase[g];
+    const uint32_t j = local / (nt + 1), k = local - j * (nt + 1);
+    lv.splits[lv.sbase[g] + (size_t)k * K + j] = k == 0 ? lv.roff[r0 + j] : lv.roff[r0 + j + 1];
+    if (j == 0 && k < nt) {
+        lv.tile_desc[lv.tbase[g] + k] = make_uint4(g, r0, K, k);
+        lv.tile_desc2[lv.tbase[g] + k] = make_uint2(lv.sbase[g] + k * K, lv.tbase[g] + g + k);
+    }
+}
+
+__device__ __forceinline__ uint64_t sat_boundary(uint64_t T0, uint64_t k, uint64_t DT) {
+    const uint64_t t = T0 + k * DT;  // k < 2^20, DT <= 2^64 / tiles: the product does not overflow
+    return t < T0 ? ~0ull : t;
+}
+
+// Tile k (of nt) of group g of level lv holds the keys in [T_k, T_k+1) (T_0 = -inf, T_nt = +inf) and owns the next
+// level's boundaries k1 = 1 .. nt1 (T1(nt1) = +inf: the run end) whose T1 lies in that range: [k_lo, k_hi).  ONE
+// thread computes the range (two 64-bit divisions) -- emit_range -- and all threads then place their boundaries --
+// emit_next_splits.
+struct EmitRange {
+    uint32_t k_lo, k_hi;  // boundaries [k_lo, k_hi) of next-level group g1
+    uint32_t g1, j1;      // next-level group and this group's run index in it
+};
+
+__device__ __forceinline__ EmitRange emit_range(const LevelDev& lv, const LevelDev& nx, uint32_t g, uint32_t k) {
+    EmitRange r;
+    r.g1 = nx.run_group[g];
+    r.j1 = g - nx.gfirst[r.g1];
+    const uint32_t nt1 = nx.tbase[r.g1 + 1] - nx.tbase[r.g1];
+    const uint32_t nt = lv.tbase[g + 1] - lv.tbase[g];
+    r.k_lo = 1; r.k_hi = 0;
+    if (nt1 == 0) return r;
+    const uint64_t T0 = lv.gT0[g], DT = lv.gDT[g], T01 = nx.gT0[r.g1], DT1 = nx.gDT[r.g1];
+    // first boundary index k1 >= 1 with T1(k1) >= T, capped at nt1 (T1(nt1) = +inf)
+    auto first_at = [&](uint64_t T) -> uint32_t {
+        if (T <= T01) return 1u;
+        const uint64_t q = (T - T01 - 1ull) / DT1 + 1ull;
+        return q < (uint64_t)nt1 ? (uint32_t)q : nt1;
+    };
+    r.k_lo = k == 0 ? 1u : first_at(sat_boundary(T0, k, DT));
+    r.k_hi = k + 1 >= nt ? nt1 + 1u : first_at(sat_boundary(T0, k + 1, DT));
+    return r;
+}
+
+// The tile's c sorted hits start at output index b0, key_at(i) is the key of the i-th; [gs, ge) is the group's output
+// range.  Called by all threads of the block with the same (block-uniform) range.
+template <class KeyAt>
+__device__ __forceinline__ void emit_next_splits(const LevelDev& nx, const EmitRange& r, uint32_t gs, uint32_t ge,
+                                                 uint32_t b0, uint32_t c, KeyAt key_at) {
+    if (r.k_lo >= r.k_hi) return;
+    const uint32_t g1 = r.g1;
+    const uint32_t K1 = nx.gfirst[g1 + 1] - nx.gfirst[g1];
+    const uint32_t nt1 = nx.tbase[g1 + 1] - nx.tbase[g1];
+    const uint64_t T01 = nx.gT0[g1], DT1 = nx.gDT[g1];
+    uint32_t* const srow = nx.splits + nx.sbase[g1] + r.j1;
+    uint32_t* const tb = nx.tile_base + nx.tbase[g1] + g1;
+    for (uint32_t k1 = r.k_lo + threadIdx.x; k1 < r.k_hi; k1 += blockDim.x) {
+        uint32_t pos = ge;
+        if (k1 < nt1) {
+            const uint64_t T = sat_boundary(T01, k1, DT1);
+            uint32_t a = 0, b = c;
+            while (a < b) { const uint32_t mid = a + ((b - a) >> 1); if (key_at(mid) < T) a = mid + 1; else b = mid; }
+            pos = b0 + a;
+            pos = pos < gs ? gs : (pos > ge ? ge : pos);  // (only unsorted runs can push it outside)
+        }
+        srow[(size_t)k1 * K1] = pos;
+        if (pos != gs) atomicAdd(tb + k1, pos - gs);
     }
 }
 
@@ -763,8 +853,8 @@ __device__ void merge_tile_general(MergeSmem& sm, const LevelDev& lv, uint32_t t
 
 // The tiles the fast kernel (tt_merge_fast.cuh) left over: a fixed grid walks the list.
 template <bool kPerm>
-__global__ void __launch_bounds__(kMThreads, 2) merge_slow_kernel(LevelDev lv, const uint4* __restrict__ in,
-                                                                  uint4* __restrict__ out,
+__global__ void __launch_bounds__(kMThreads, 2) merge_slow_kernel(LevelDev lv, LevelDev nx, int has_next,
+                                                                  const uint4* __restrict__ in, uint4* __restrict__ out,
                                                                   const uint32_t* __restrict__ perm_in,
                                                                   uint32_t* __restrict__ perm_out, int check_runs,
                                                                   int32_t* __restrict__ status) {
@@ -775,8 +865,20 @@ __global__ void __launch_bounds__(kMThreads, 2) merge_slow_kernel(LevelDev lv, c
     if (threadIdx.x == 0) mbar_init(&sm.mbar, 1);
     uint32_t phase = 0;
     for (uint32_t i = blockIdx.x; i < n_slow; i += gridDim.x) {
-        merge_tile_general<kPerm>(sm, lv, lv.slow_list[i], in, out, perm_in, perm_out, check_runs, status, phase);
-        __syncthreads();
+        const uint32_t tile = lv.slow_list[i];
+        merge_tile_general<kPerm>(sm, lv, tile, in, out, perm_in, perm_out, check_runs, status, phase);
+        __syncthreads();  // the tile is in global memory, visible to this block
+        if (has_next) {
+            const uint4 td = lv.tile_desc[tile];
+            const uint2 td2 = lv.tile_desc2[tile];
+            const uint32_t gs = lv.roff[td.y], ge = lv.roff[td.y + td.z];
+            uint32_t b0 = gs + lv.tile_base[td2.y], b1 = gs + lv.tile_base[td2.y + 1];
+            b0 = b0 > ge ? ge : b0;
+            b1 = b1 > ge ? ge : (b1 < b0 ? b0 : b1);
+            const uint4* o = out;
+            const EmitRange er = emit_range(lv, nx, td.x, td.w);  // (every thread: the general path is rare)
+            emit_next_splits(nx, er, gs, ge, b0, b1 - b0, [&](uint32_t q) { return key_of(hit_time(__ldcg(o + b0 + q))); });
+        }
     }
 }
 
@@ -889,6 +991,8 @@ static void carve(Arena& a, const std::vector<LevelHost>& levels, uint32_t n, bo
         d.sbase = a.take<uint32_t>(L.G + 1);
         d.gT0 = a.take<uint64_t>(L.G + 1);
         d.gDT = a.take<uint64_t>(L.G + 1);
+        d.gKmax = a.take<uint64_t>(L.G + 1);
+        d.run_group = a.take<uint32_t>((size_t)L.R + 1);
         d.gScale = a.take<uint32_t>(L.G + 1);
         d.splits = a.take<uint32_t>((size_t)L.split_entries + 1);
         d.roff_next = a.take<uint32_t>(L.G + 1);
@@ -941,6 +1045,7 @@ int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_
     const uint32_t* psrc = nullptr;
     FuseL1 none;
     none.flags = nullptr; none.lc = 0; none.q_thresh = 0;
+    bool planned = false;  // this level's plan and split table were made by the previous level (emit_next_splits)
     for (size_t l = 0; l < nlev; ++l) {
         LevelDev& d = w.dev[l];
         d.roff = l == 0 ? d_run_offsets : w.dev[l - 1].roff_next;
@@ -948,29 +1053,45 @@ int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_
         const bool fused = is_last && fuse && fuse->flags;
         uint4* dst = is_last ? (uint4*)d_out : w.tmp[l & 1];
         uint32_t* pdst = d_perm ? (is_last ? d_perm : w.ptmp[l & 1]) : nullptr;
-        prof_mark(s, l == 0 ? "sort.merge_plan0" : "sort.merge_plan1");
-        TT_K(merge_groups_kernel)<<<1, 1024, 0, s>>>(d, d_seg_offsets, n_seg);
-        TT_K(merge_setup_kernel)<<<1, 1024, 0, s>>>(d, src, n);
-        TT_CUDA_OK(cudaMemsetAsync(d.tile_base, 0, ((size_t)levels[l].tiles + levels[l].G + 2) * sizeof(uint32_t), s));
-        if (levels[l].split_entries) {
-            prof_mark(s, l == 0 ? "sort.merge_partition0" : "sort.merge_partition1");
-            if (levels[l].kmax >= kInterpFan)
-                TT_K(merge_partition_kernel<true>)<<<div_up(levels[l].split_entries, 256), 256, 0, s>>>(d, src, levels[l].split_entries);
-            else
-                TT_K(merge_partition_kernel<false>)<<<div_up(levels[l].split_entries, 256), 256, 0, s>>>(d, src, levels[l].split_entries);
+        if (!planned) {
+            prof_mark(s, l == 0 ? "sort.merge_plan0" : "sort.merge_plan1");
+            TT_K(merge_groups_kernel)<<<1, 1024, 0, s>>>(d, d_seg_offsets, n_seg);
+            TT_K(merge_setup_kernel)<<<1, 1024, 0, s>>>(d, src, n, nullptr, nullptr);
+            TT_CUDA_OK(cudaMemsetAsync(d.tile_base, 0, ((size_t)levels[l].tiles + levels[l].G + 2) * sizeof(uint32_t), s));
+            if (levels[l].split_entries) {
+                prof_mark(s, l == 0 ? "sort.merge_partition0" : "sort.merge_partition1");
+                if (levels[l].kmax >= kInterpFan)
+                    TT_K(merge_partition_kernel<true>)<<<div_up(levels[l].split_entries, 256), 256, 0, s>>>(d, src, levels[l].split_entries);
+                else
+                    TT_K(merge_partition_kernel<false>)<<<div_up(levels[l].split_entries, 256), 256, 0, s>>>(d, src, levels[l].split_entries);
+            }
         }
+        // the next level's plan, from this level's group key ranges, BEFORE this level's tiles run: they fill its split table
+        const bool emit = !is_last && levels[l].tiles && levels[l + 1].split_entries;
+        LevelDev nx = d;
+        if (emit) {
+            LevelDev& e = w.dev[l + 1];
+            e.roff = d.roff_next;
+            prof_mark(s, "sort.merge_plan1");
+            TT_K(merge_groups_kernel)<<<1, 1024, 0, s>>>(e, d_seg_offsets, n_seg);
+            TT_K(merge_setup_kernel)<<<1, 1024, 0, s>>>(e, nullptr, n, d.gT0, d.gKmax);
+            TT_CUDA_OK(cudaMemsetAsync(e.tile_base, 0, ((size_t)levels[l + 1].tiles + levels[l + 1].G + 2) * sizeof(uint32_t), s));
+            TT_K(merge_init_next_kernel)<<<div_up(levels[l + 1].split_entries, 256), 256, 0, s>>>(e, levels[l + 1].split_entries);
+            nx = e;
+        }
+        planned = emit;
         if (levels[l].tiles) {
             prof_mark(s, l == 0 ? "sort.merge_tile0" : "sort.merge_tile1");
             const uint32_t nt = levels[l].tiles;
-            const int chk = l == 0;
+            const int chk = l == 0, hn = emit ? 1 : 0;
             if (d_perm) {
-                if (fused) TT_K((merge_fast_kernel<true, true>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, src, dst, psrc, pdst, chk, *fuse, d_status);
-                else TT_K((merge_fast_kernel<true, false>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, src, dst, psrc, pdst, chk, none, d_status);
-                TT_K(merge_slow_kernel<true>)<<<slow_grid, kMThreads, sizeof(MergeSmem), s>>>(d, src, dst, psrc, pdst, chk, d_status);
+                if (fused) TT_K((merge_fast_kernel<true, true>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, nx, hn, src, dst, psrc, pdst, chk, *fuse, d_status);
+                else TT_K((merge_fast_kernel<true, false>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, nx, hn, src, dst, psrc, pdst, chk, none, d_status);
+                TT_K(merge_slow_kernel<true>)<<<slow_grid, kMThreads, sizeof(MergeSmem), s>>>(d, nx, hn, src, dst, psrc, pdst, chk, d_status);
             } else {
-                if (fused) TT_K((merge_fast_kernel<false, true>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, src, dst, nullptr, nullptr, chk, *fuse, d_status);
-                else TT_K((merge_fast_kernel<false, false>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, src, dst, nullptr, nullptr, chk, none, d_status);
-                TT_K(merge_slow_kernel<false>)<<<slow_grid, kMThreads, sizeof(MergeSmem), s>>>(d, src, dst, nullptr, nullptr, chk, d_status);
+                if (fused) TT_K((merge_fast_kernel<false, true>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, nx, hn, src, dst, nullptr, nullptr, chk, *fuse, d_status);
+                else TT_K((merge_fast_kernel<false, false>))<<<nt, kFThreads, sizeof(FastSmem), s>>>(d, nx, hn, src, dst, nullptr, nullptr, chk, none, d_status);
+                TT_K(merge_slow_kernel<false>)<<<slow_grid, kMThreads, sizeof(MergeSmem), s>>>(d, nx, hn, src, dst, nullptr, nullptr, chk, d_status);
             }
         }
         if (is_last && last) { last->lv = d; last->tiles = levels[l].tiles; }

@@ -12,6 +12,8 @@ struct LevelDev {
     uint32_t* sbase;         // [G+1] exclusive prefix of split-table entries per group ((tiles+1) * K)
     uint64_t* gT0;           // [G] smallest key of the group
     uint64_t* gDT;           // [G] tile width in key units (>= 1)
+    uint64_t* gKmax;         // [G] largest key of the group
+    uint32_t* run_group;     // [R] group of every run of this level
     uint32_t* gScale;        // [G] floor(kFCap * 2^32 / DT) when kFCap < DT < 2^32 (the fast tile kernel's bucket map), else 0
     uint32_t* splits;        // split table
     uint32_t* roff_next;     // [G+1] run offsets of the next level (= group boundaries)

@@ -29,6 +29,7 @@ struct FastSmem {
     uint32_t cur[kMaxFan];           // absolute index of the first hit of every piece
     uint32_t pstart[kFCap / 32];     // bitmap of piece starts (run-order check)
     uint32_t scan[64];
+    uint32_t emit[4];                // EmitRange of this tile (thread kFThreads - 1 computes it while the tile is loading)
     uint64_t mbar;
 };
 static_assert(2 * (sizeof(FastSmem) + 1024) <= 233472, "two CTAs per SM");
@@ -48,8 +49,8 @@ __device__ __forceinline__ uint64_t tile_key(const uint4* tile, uint32_t e) {
 }
 
 template <bool kPerm, bool kFuse>
-__global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, const uint4* __restrict__ in,
-                                                                  uint4* __restrict__ out,
+__global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, LevelDev nx, int has_next,
+                                                                  const uint4* __restrict__ in, uint4* __restrict__ out,
                                                                   const uint32_t* __restrict__ perm_in,
                                                                   uint32_t* __restrict__ perm_out, int check_runs,
                                                                   FuseL1 fz, int32_t* __restrict__ status) {
@@ -84,8 +85,12 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, c
     const uint32_t my_s0 = block_scan1(my_len, sm.scan, &total);  // one barrier (orders the clearing above too)
     if (total == 0 || total > (uint32_t)kFCap || scale == 0u || out_base > out_end) {
         if (tid == 0) {
-            if (total) lv.slow_list[atomicAdd(lv.slow_cnt, 1u)] = blockIdx.x;
+            if (total) lv.slow_list[atomicAdd(lv.slow_cnt, 1u)] = blockIdx.x;  // merge_slow_kernel sorts it (and emits)
             if (kFuse) lv.tile_open[blockIdx.x] = total ? 1 : 0;
+        }
+        if (!kFuse && has_next && total == 0) {  // an empty tile still owns the next level's boundaries of its key range
+            const EmitRange er = emit_range(lv, nx, g, k);
+            emit_next_splits(nx, er, lv.roff[r0], out_end, min(out_base, out_end), 0u, [](uint32_t) { return 0ull; });
         }
         return;
     }
@@ -108,6 +113,10 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, c
             const uint32_t s0 = sm.segstart[jj], len = sm.segstart[jj + 1] - s0;
             if (len) bulk_g2s(&sm.tile[s0], in + sm.cur[jj], len * 16u, &sm.mbar);
         }
+    }
+    if (!kFuse && has_next && tid == kFThreads - 1) {  // while the tile is on its way; read after later barriers
+        const EmitRange er = emit_range(lv, nx, g, k);
+        sm.emit[0] = er.k_lo; sm.emit[1] = er.k_hi; sm.emit[2] = er.g1; sm.emit[3] = er.j1;
     }
     uint64_t Ta = T0 + (uint64_t)k * DT;
     if (Ta < T0) Ta = ~0ull;
@@ -224,6 +233,11 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, c
     __syncthreads();
     const uint32_t n_store = min(total, out_end - out_base);
     if (tid == 0 && n_store) bulk_s2g(out + out_base, sm.tile, n_store * 16u);
+    if (!kFuse && has_next) {  // the next level's split rows from the sorted tile (see emit_next_splits in tt_merge.cu)
+        EmitRange er;
+        er.k_lo = sm.emit[0]; er.k_hi = sm.emit[1]; er.g1 = sm.emit[2]; er.j1 = sm.emit[3];
+        emit_next_splits(nx, er, lv.roff[r0], out_end, out_base, total, [&](uint32_t q) { return tile_key(sm.tile, q); });
+    }
     if (kPerm) {
         for (uint32_t r = tid; r < n_store; r += kFThreads) perm_out[out_base + r] = sm.list[r];
         if (kFuse) __syncthreads();  // list is reused below
