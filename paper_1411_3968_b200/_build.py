@@ -27,7 +27,7 @@ def stale() -> bool:
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
         nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-        cmd = [nvcc, *NVCC_FLAGS, "-o", LIB, *sources()]
+        cmd = [nvcc, *NVCC_FLAGS, *os.environ.get("TT_NVCC_EXTRA", "").split(), "-o", LIB, *sources()]
         if verbose:
             print(" ".join(cmd))
         subprocess.check_call(cmd)
