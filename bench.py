@@ -489,15 +489,29 @@ def run_ours(args):
     if rank == 0:
         l0_n, l0_tw = 7, (1_000_000 if args.config == 0 else 500_000)
         g_multi = w.geometry.n_tower > 1
+        l0_src, l0_seg, l0_scope = d_out, seg, "the sorted slice"
+        ppt_ = w.geometry.pmts_per_tower
+        if g_multi and (len(w.run_offsets) - 1) % ppt_ == 0:
+            # The paper applies N7TW500, SC, FC and AFC PER TOWER.  On the time-merged stream of 100
+            # towers every window fires and a hit walks the hits of 99 foreign towers, so these legs run on the
+            # per-tower streams instead: the same input sorted with one segment per (slice, tower) -- the runs are
+            # tower-major, so a tower's 84 runs are contiguous -- and windows / pairs never cross a segment.
+            l0_seg = B.Offsets(np.ascontiguousarray(w.run_offsets[::ppt_], dtype=np.uint32))
+            l0_src = torch.empty_like(run.d_in)
+            st_ = torch.zeros(1, dtype=torch.int32, device="cuda")
+            B.tt_sort_slice(run.d_in, l0_src, None, l0_seg, runs, st_)
+            torch.cuda.synchronize()
+            assert int(st_.item()) == 0
+            l0_scope = f"per-tower streams: {l0_seg.count} segments of one (slice, tower) each, sorted by tt_sort_slice"
         d_l0 = torch.empty(n, dtype=torch.uint8, device="cuda")
         d_l0n = torch.zeros(1, dtype=torch.int32, device="cuda")
         for _ in range(3):
-            B.tt_l0_ntw(d_out, seg, l0_n, l0_tw, d_l0, d_l0n)
+            B.tt_l0_ntw(l0_src, l0_seg, l0_n, l0_tw, d_l0, d_l0n)
         torch.cuda.synchronize()
         a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a0.record()
         for _ in range(args.steps):
-            B.tt_l0_ntw(d_out, seg, l0_n, l0_tw, d_l0, d_l0n)
+            B.tt_l0_ntw(l0_src, l0_seg, l0_n, l0_tw, d_l0, d_l0n)
         a1.record()
         torch.cuda.synchronize()
         l0_ms = a0.elapsed_time(a1) / args.steps
@@ -505,11 +519,8 @@ def run_ours(args):
         l0 = {"kernel": "l0_ntw_kernel", "multiplicity": l0_n, "window_ps": l0_tw, "ms": l0_ms,
               "hits_per_s": n / (l0_ms * 1e-3), "alg_bytes_per_hit": 17, "achieved": l0_ach, "peak": peak,
               "unit": "GB/s", "frac": l0_ach / peak, "n_start": int(d_l0n.cpu().numpy().view(np.uint32)[0]),
-              "note": ("level-0 / DN / pair / combine legs: separate calls on the sorted hits, outside the timed step.  "
-                       "The paper applies N7TW500, SC, FC and AFC per 84-PMT tower; on the multi-tower stream of "
-                       "cfg4 (100 towers superimposed, 462 hits/us) every window start fires, so these cfg4 "
-                       "figures are BANDWIDTH PROBES of the kernels, not trigger results") if g_multi else
-                      "separate calls on the sorted hits, outside the timed step"}
+              "scope": l0_scope,
+              "note": "level-0 / DN / pair / combine legs: separate calls, outside the timed step"}
         # the paper's pair seeds (SC / FC / AFC) and its combination with the level-0 windows
         # (PAPER.md:65, 73): tt_pair_seeds 16 B read + 1 B written per hit, tt_l0_combine 2 B read + 1 B written
         gw = w.geometry
@@ -530,7 +541,7 @@ def run_ours(args):
             return b0.elapsed_time(b1) / reps
 
         reps = max(2, min(args.steps, 5))
-        ps_ms = timed(lambda: B.tt_pair_seeds(d_out, seg, d_adj, gw.pmts_per_tower, d_pb), reps)
+        ps_ms = timed(lambda: B.tt_pair_seeds(l0_src, l0_seg, d_adj, gw.pmts_per_tower, d_pb), reps)
         cb_ms = timed(lambda: B.tt_l0_combine(d_l0, d_pb, n, l0_n, d_cd, d_nc), reps)
         nc = d_nc.cpu().numpy().view(np.uint32)
         l0["pair_seeds"] = {"kernel": "pair_seeds_kernel", "windows_ps": [20_000, 100_000, 250_000], "ms": ps_ms,
@@ -542,12 +553,12 @@ def run_ours(args):
         # distinct-PMT variant DN7: 16 B read + 1 B zeroed + 1 B written per hit
         d_dn = torch.empty(n, dtype=torch.uint8, device="cuda")
         d_dnn = torch.zeros(1, dtype=torch.int32, device="cuda")
-        dn_ms = timed(lambda: B.tt_l0_dntw(d_out, seg, l0_n, l0_tw, d_dn, d_dnn), reps)
+        dn_ms = timed(lambda: B.tt_l0_dntw(l0_src, l0_seg, l0_n, l0_tw, d_dn, d_dnn), reps)
         l0["dn"] = {"kernel": "l0_dntw_kernel", "multiplicity": l0_n, "window_ps": l0_tw, "ms": dn_ms,
                     "alg_bytes_per_hit": 18, "achieved": 18.0 * n / (dn_ms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
                     "frac": 18.0 * n / (dn_ms * 1e-3) / 1e9 / peak,
                     "n_start": int(d_dnn.cpu().numpy().view(np.uint32)[0])}
-        del d_l0, d_pb, d_cd, d_dn
+        del d_l0, d_pb, d_cd, d_dn, l0_src
 
     # ---- end to end through the C ABI with host buffers (pinned), copies inside the timed region ----
     e2e = None

@@ -26,6 +26,8 @@ struct DnSmem {
     uint32_t f[kDTile / 4];  // result bytes of the tile
     uint16_t seen[TT_MAX_DN_MULTIPLICITY][kDThreads];  // the different PMTs of the running window, one column per thread
     uint32_t red[kDThreads / 32];
+    uint32_t n_cand;                // starts that passed the plain N-in-TW pre-test
+    uint16_t cand[kDTile];          // their tile positions
 };
 
 // OR `bits` into byte i of a byte array of any alignment (the aligned 32-bit word around it lies inside the same
@@ -65,19 +67,39 @@ __global__ void __launch_bounds__(kDThreads) l0_dntw_kernel(const uint4* __restr
         sm.pmt[q] = (uint16_t)p;
     }
     sm.f[tid] = 0;
+    if (tid == 0) sm.n_cand = 0;
     __syncthreads();
-    uint32_t my_starts = 0;
-#pragma unroll 1
+    // N different PMTs need N hits: the plain N-in-TW test on hit k + N - 1 (staged: N - 1 < kDHalo) rules out most
+    // starts of a quiet tower before any scan (one tower at 55 kHz per PMT: 97 %).  The survivors go to a list and are
+    // scanned one per thread afterwards, so a warp is not held by the one lane in thirty that has a window to walk.
+#pragma unroll
     for (int r = 0; r < kDPer; ++r) {
         const uint32_t q = tid + r * kDThreads;
         const uint32_t k = tb + q;
-        if (k >= te) break;
+        bool pass = false;
+        if (k < te) {
+            uint32_t sb = seg_b;
+            if (!one_seg) sb = __ldg(seg_off + find_segment(seg_off, n_seg, k) + 1);
+            pass = (uint64_t)k + N - 1 < sb && sm.key[q + N - 1] - sm.key[q] < tw;
+        }
+        const uint32_t mk = __ballot_sync(0xffffffffu, pass);
+        if (mk) {
+            uint32_t base = 0;
+            if ((tid & 31u) == 0) base = atomicAdd(&sm.n_cand, (uint32_t)__popc(mk));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (pass) sm.cand[base + (uint32_t)__popc(mk & lanemask_lt())] = (uint16_t)q;
+        }
+    }
+    __syncthreads();
+    const uint32_t n_cand = sm.n_cand;
+    uint32_t my_starts = 0;
+#pragma unroll 1
+    for (uint32_t c = tid; c < n_cand; c += kDThreads) {
+        const uint32_t q = sm.cand[c];
+        const uint32_t k = tb + q;
         uint32_t sb = seg_b;
         if (!one_seg) sb = __ldg(seg_off + find_segment(seg_off, n_seg, k) + 1);
         const uint64_t tk = sm.key[q];
-        // N different PMTs need N hits: the plain N-in-TW test on hit k + N - 1 (staged: N - 1 < kDHalo) rules out most
-        // starts of a quiet tower before any scan
-        if ((uint64_t)k + N - 1 >= sb || sm.key[q + N - 1] - tk >= tw) continue;
         // the different PMTs seen so far: a 64-bit Bloom mask in a register decides "new" in the common case, the exact
         // list (a column of shared memory) is only read when the mask bit is already set
         uint64_t mask = 0;
