@@ -1129,7 +1129,7 @@ static int trigger_run(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg
     TT_K(l2_clique_kernel)<<<sms * 6, kClqTile, 0, s>>>(plan.l1, plan.m_total, plan.rows, p->l2_multiplicity, p->l2_mode,
                                                         d_flags, plan.l2bit, plan.slow_list, plan.slow_cnt);
     prof_mark(s, "trig.l2_wide");
-    TT_K(l2_wide_kernel)<<<sms * 4, kL2Warps * 32, sizeof(WideSmem) * kL2Warps, s>>>(
+    TT_K(l2_wide_kernel)<<<sms * 12, kL2Warps * 32, sizeof(WideSmem) * kL2Warps, s>>>(
         plan.l1, plan.m_total, plan.slow_list, plan.slow_cnt, d_seg_offsets, n_seg, n, g->dev, (uint64_t)p->l2_window_ps,
         p->l2_multiplicity, p->l2_mode, d_flags, plan.l2bit, d_status);
     prof_counter(s, "l1_hits", plan.m_total);

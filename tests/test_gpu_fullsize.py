@@ -1,5 +1,6 @@
-"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (three calls, INEVT
-tagging, seed / event capacity n / 4), on all five configs (north_star: "GPU output bit-exact with the oracle on all
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (tt_sort_trigger_slice +
+tt_extract_events with INEVT tagging, seed / event capacity n / 4; the three separate calls are run too and must give
+the same bytes), on all five configs (north_star: "GPU output bit-exact with the oracle on all
 five configs").
 
 Three layers, cheapest first:
@@ -48,8 +49,9 @@ def _run_bench_config(B, w):
     d_seeds = torch.zeros(cap, dtype=torch.int32, device="cuda")
     d_ev = torch.zeros((cap, 4), dtype=torch.int64, device="cuda")
     d_cnt = torch.zeros(4, dtype=torch.int32, device="cuda")
-    B.tt_sort_slice(d_in, d_out, None, seg, runs, d_cnt[2:3])
-    B.tt_trigger_slice(d_out, seg, geo, prm, d_flags, d_seeds, d_cnt[0:1], d_cnt[2:3])
+    # bench.py's step: the fused call + events
+    d_flags.fill_(0xEE)  # every byte is written by the fused call
+    B.tt_sort_trigger_slice(d_in, d_out, None, seg, runs, geo, prm, d_flags, d_seeds, d_cnt[0:1], d_cnt[2:3])
     B.tt_extract_events(d_out, seg, d_seeds, d_cnt[0:1], prm, d_ev, d_cnt[1:2], d_flags, None, None, d_cnt[2:3])
     torch.cuda.synchronize()
     cnt = d_cnt.cpu().numpy().view(np.uint32)
@@ -59,6 +61,18 @@ def _run_bench_config(B, w):
     flags = d_flags.cpu().numpy()
     seeds = d_seeds[:ns].cpu().numpy().view(np.uint32)
     events = d_ev[:ne].cpu().numpy().reshape(-1).view(B.EVENT_DTYPE).copy()
+    # the three separate calls (bench.py --fused off) give the same bytes
+    d_cnt.zero_(); d_out.fill_(-1); d_flags.fill_(0); d_seeds.fill_(-1); d_ev.fill_(-1)
+    B.tt_sort_slice(d_in, d_out, None, seg, runs, d_cnt[2:3])
+    B.tt_trigger_slice(d_out, seg, geo, prm, d_flags, d_seeds, d_cnt[0:1], d_cnt[2:3])
+    B.tt_extract_events(d_out, seg, d_seeds, d_cnt[0:1], prm, d_ev, d_cnt[1:2], d_flags, None, None, d_cnt[2:3])
+    torch.cuda.synchronize()
+    cnt3 = d_cnt.cpu().numpy().view(np.uint32)
+    assert (int(cnt3[0]), int(cnt3[1]), int(cnt3[2])) == (ns, ne, status), "three calls and fused call: counts differ"
+    assert torch.equal(d_flags, torch.from_numpy(flags).cuda()), "three calls and fused call: flags differ"
+    assert B.hits_to_host(d_out).tobytes() == srt.tobytes(), "three calls and fused call: sorted records differ"
+    assert (d_seeds[:ns].cpu().numpy().view(np.uint32) == seeds).all(), "three calls and fused call: seeds differ"
+    assert d_ev[:ne].cpu().numpy().reshape(-1).view(B.EVENT_DTYPE).tobytes() == events.tobytes(), "events differ"
     del d_flags, d_seeds, d_ev
     # the permutation output (bench.py does not ask for it): a second sort call into a scratch buffer
     d_out.fill_(-1)
