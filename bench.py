@@ -271,12 +271,12 @@ def time_radix(B, run, peak):
 
 def time_prepare(B, peak):
     """tt_prepare_slice (NEXT-3) on the raw stream of a cfg2-shaped burst: five 200 ms sub-slices at
-    one tenth of the duration (3 M raw hits, 28 B each on average) -> PMT-major 16-byte records + run offsets."""
+    half the duration (15 M raw hits, 28 B each on average) -> PMT-major 16-byte records + run offsets."""
     import torch
 
     from paper_1411_3968_b200 import workload as W
 
-    w = W.make_config(2, time_scale=0.1)
+    w = W.make_config(2, time_scale=0.5)
     raw, samples, slice_off = W.make_raw(w)
     n = len(raw)
     d_raw = torch.from_numpy(raw.view(np.int64).reshape(-1, 2).copy()).cuda()
@@ -293,7 +293,7 @@ def time_prepare(B, peak):
     ms = _cuda_time(go, 5)
     assert B.hits_to_host(d_out).tobytes() == np.ascontiguousarray(w.hits).tobytes(), "prepare differs from the generator"
     byt = raw.nbytes + samples.nbytes + 16 * n
-    return {"workload": w.name + " x 0.1", "raw_hits": n, "raw_bytes_per_hit": (raw.nbytes + samples.nbytes) / n,
+    return {"workload": w.name + " x 0.5", "raw_hits": n, "raw_bytes_per_hit": (raw.nbytes + samples.nbytes) / n,
             "ms": ms, "hits_per_s": n / (ms * 1e-3), "alg_bytes": byt, "frac": byt / (ms * 1e-3) / 1e9 / peak,
             "paper": "200-300 ms of CPU time per second of data, transfer included (PAPER.md:71)"}
 
