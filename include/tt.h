@@ -81,6 +81,7 @@ enum {
     TT_S_EVENT_OVERFLOW = 2, /* likewise for events                                                   */
     TT_S_RUN_UNSORTED = 4,   /* a run given by d_run_offsets is not non-decreasing: output unspecified */
     TT_S_BAD_PMT = 8,        /* an L1 hit has pmt_id >= n_pmt (it has no L2 edges)                     */
+    TT_S_L1_OVERFLOW = 64,   /* tt_l1_export: more L1 hits than l1_cap (*d_n_l1 is the true count, first l1_cap valid)   */
     TT_S_RAW_TRUNCATED = 32, /* tt_prepare_slice: a waveform reaches behind the sample section (missing samples = 0) */
     TT_S_DENSITY = 16        /* an L1 hit has more than TT_MAX_NEIGHBOURS L1 hits of its segment within
                                 +-min(W, largest table entry) of it: its L2STAR bit is exact, and its
@@ -222,6 +223,45 @@ int tt_prepare_slice(const tt_raw_hit* d_raw, const uint16_t* d_samples, uint32_
                      const uint32_t* d_slice_offsets, const uint32_t* h_slice_offsets, uint32_t n_slices,
                      uint32_t n_pmt, tt_hit* d_out, uint32_t out_cap, uint32_t* d_run_offsets, void* d_ws,
                      size_t* ws_bytes, int32_t* d_status, void* stream);
+
+/* ---- A multi-tower detector sharded BY TOWER over several GPUs, with one exchange (
+ * PAPER.md:81, sect. 5: "each TGPU finds the trigger seeds of its tower and sends them to a TCPU ... gets candidate
+ * times back").  L1 is local to a floor, hence to a tower; only L2 and the event windows look across towers.  Per rank
+ * (a contiguous range of towers; pmt ids and floor ids stay GLOBAL):
+ *   tt_sort_l1_slice   its hits -> time-sorted + Q / LC / L1 flag bytes (tt_sort_trigger_slice without L2 / seeds;
+ *                      runs required);
+ *   tt_l1_export       its L1 hits, in sorted order, as 16-byte records {t_ps, idx = sorted index, pmt_id, src = rank};
+ *   -- the ranks all-gather their records (NCCL; ~2 % of the hits) and concatenate them in rank order --
+ *   tt_sort_slice      on the concatenation (one run per rank; the record starts with the time, like a hit) merges it;
+ *   tt_l2_merged       L2STAR / L2 of every record of the merged list (the L2 kernels of tt_trigger_slice; same
+ *                      geometry, same status bits) into d_bits[m], and the positions of the L2 records -- the GLOBAL
+ *                      seed list, identical on every rank -- into d_seeds;
+ *   tt_extract_events  on (merged list as hits, d_seeds) gives the global event windows (t_start, t_end, seed_begin,
+ *                      n_seeds as on one GPU; hit_begin / hit_end index the merged list);
+ *   tt_l2_apply        writes the L2STAR / L2 bits of the rank's own records into its flag bytes and its own seeds
+ *                      (ascending sorted indices) into d_seeds;
+ *   tt_tag_windows     ORs TT_INEVT into the flags of the rank's hits inside any of the global windows.
+ * Flags, seeds (per rank) and window times then equal, hit for hit, what one GPU computes on the whole detector.
+ * Workspace / status / stream conventions as above. */
+typedef struct {
+    int64_t t_ps;
+    uint32_t idx;
+    uint16_t pmt_id, src;
+} tt_l1hit;
+int tt_sort_l1_slice(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n, const uint32_t* d_seg_offsets,
+                     const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* d_run_offsets,
+                     const uint32_t* h_run_offsets, uint32_t n_runs, const tt_params* p, uint8_t* d_flags, void* d_ws,
+                     size_t* ws_bytes, int32_t* d_status, void* stream);
+int tt_l1_export(const tt_hit* d_sorted, uint32_t n, const uint8_t* d_flags, uint32_t src, tt_l1hit* d_l1, uint32_t l1_cap,
+                 uint32_t* d_n_l1, void* d_ws, size_t* ws_bytes, int32_t* d_status, void* stream);
+int tt_l2_merged(const tt_l1hit* d_l1, uint32_t m, const tt_geometry* g, const tt_params* p, uint8_t* d_bits,
+                 uint32_t* d_seeds, uint32_t seed_cap, uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes,
+                 int32_t* d_status, void* stream);
+int tt_l2_apply(const tt_l1hit* d_l1, const uint8_t* d_bits, uint32_t m, uint32_t src, uint8_t* d_flags, uint32_t n,
+                uint32_t* d_seeds, uint32_t seed_cap, uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes,
+                int32_t* d_status, void* stream);
+int tt_tag_windows(const tt_hit* d_sorted, uint32_t n, const tt_event* d_events, const uint32_t* d_n_events,
+                   uint32_t event_cap, const tt_params* p, uint8_t* d_flags, void* stream);
 
 /* Whole-slice convenience with HOST buffers (end-to-end use and timing; not a hot call).
  * tt_host_ctx_create allocates, once, device buffers and workspaces for slices of up to max_n hits,

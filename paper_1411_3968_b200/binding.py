@@ -21,12 +21,13 @@ TT_Q, TT_LC, TT_L1, TT_L2STAR, TT_L2, TT_INEVT = 1, 2, 4, 8, 16, 32
 TT_OK, TT_E_INVAL, TT_E_CUDA, TT_E_WORKSPACE = 0, -1, -2, -3
 TT_S_SEED_OVERFLOW, TT_S_EVENT_OVERFLOW, TT_S_RUN_UNSORTED, TT_S_BAD_PMT, TT_S_DENSITY = 1, 2, 4, 8, 16
 TT_S_RAW_TRUNCATED = 32
+TT_S_L1_OVERFLOW = 64
 
 EXPORTS = ["tt_version", "tt_geometry_create", "tt_geometry_destroy", "tt_sort_slice", "tt_trigger_slice",
            "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host", "tt_launch_count",
            "tt_prof_enable", "tt_prof_read", "tt_l0_ntw", "tt_pair_seeds", "tt_l0_combine",
            "tt_l0_dntw", "tt_sort_trigger_slice", "tt_prepare_slice", "tt_host_submit",
-           "tt_host_wait"]
+           "tt_host_wait", "tt_sort_l1_slice", "tt_l1_export", "tt_l2_merged", "tt_l2_apply", "tt_tag_windows"]
 
 HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
 EVENT_DTYPE = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
@@ -266,6 +267,55 @@ def tt_extract_events(d_sorted: torch.Tensor, seg: Offsets, d_seeds: torch.Tenso
 
 
 RAW_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("n_samples", "<u2"), ("pad", "<u2")])
+L1HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("idx", "<u4"), ("pmt_id", "<u2"), ("src", "<u2")])
+
+
+# ---- the by-tower sharded trigger (include/tt.h: NEXT-4).  Records are (m, 2) int64 CUDA tensors (16 bytes each).
+def _ws_call(call, what, ws):
+    if ws is None:
+        ws = _ws(call, what)
+    nb = c_sz(ws.numel())
+    _check(call(_dp(ws), ctypes.byref(nb)), what)
+    return ws
+
+
+def tt_sort_l1_slice(d_in, d_out, d_perm, seg: Offsets, runs: Offsets, params: TTParams, d_flags, d_status, ws=None):
+    _need_cuda()
+    L, n = load(), d_in.shape[0]
+    return _ws_call(lambda w, nb: L.tt_sort_l1_slice(_dp(d_in), _dp(d_out), _dp(d_perm), c_u32(n), _dp(seg.d), _hp(seg.h),
+                                                     c_u32(seg.count), _dp(runs.d), _hp(runs.h), c_u32(runs.count),
+                                                     ctypes.byref(params), _dp(d_flags), w, nb, _dp(d_status), _stream()),
+                    "tt_sort_l1_slice", ws)
+
+
+def tt_l1_export(d_sorted, d_flags, src: int, d_l1, d_n_l1, d_status, ws=None):
+    _need_cuda()
+    L, n = load(), d_sorted.shape[0]
+    return _ws_call(lambda w, nb: L.tt_l1_export(_dp(d_sorted), c_u32(n), _dp(d_flags), c_u32(int(src)), _dp(d_l1),
+                                                 c_u32(d_l1.shape[0]), _dp(d_n_l1), w, nb, _dp(d_status), _stream()),
+                    "tt_l1_export", ws)
+
+
+def tt_l2_merged(d_l1, geo: Geometry, params: TTParams, d_bits, d_seeds, d_n_seeds, d_status, ws=None):
+    _need_cuda()
+    L, m = load(), d_l1.shape[0]
+    return _ws_call(lambda w, nb: L.tt_l2_merged(_dp(d_l1), c_u32(m), geo.handle, ctypes.byref(params), _dp(d_bits),
+                                                 _dp(d_seeds), c_u32(d_seeds.numel()), _dp(d_n_seeds), w, nb,
+                                                 _dp(d_status), _stream()), "tt_l2_merged", ws)
+
+
+def tt_l2_apply(d_l1, d_bits, src: int, d_flags, n: int, d_seeds, d_n_seeds, d_status, ws=None):
+    _need_cuda()
+    L, m = load(), d_l1.shape[0]
+    return _ws_call(lambda w, nb: L.tt_l2_apply(_dp(d_l1), _dp(d_bits), c_u32(m), c_u32(int(src)), _dp(d_flags), c_u32(n),
+                                                _dp(d_seeds), c_u32(d_seeds.numel()), _dp(d_n_seeds), w, nb, _dp(d_status),
+                                                _stream()), "tt_l2_apply", ws)
+
+
+def tt_tag_windows(d_sorted, d_events, d_n_events, params: TTParams, d_flags):
+    _need_cuda()
+    _check(load().tt_tag_windows(_dp(d_sorted), c_u32(d_sorted.shape[0]), _dp(d_events), _dp(d_n_events),
+                                 c_u32(d_events.shape[0]), ctypes.byref(params), _dp(d_flags), _stream()), "tt_tag_windows")
 
 
 def tt_prepare_slice(d_raw: torch.Tensor, d_samples: torch.Tensor, slices: Offsets, n_pmt: int, d_out: torch.Tensor,

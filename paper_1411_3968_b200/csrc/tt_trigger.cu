@@ -1089,6 +1089,10 @@ static int trigger_args_ok(uint32_t n, const uint32_t* h_seg_offsets, uint32_t n
     return TT_OK;
 }
 
+static int trigger_l2(const TriggerPlan& plan, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
+                      const tt_geometry* g, const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds, uint32_t seed_cap,
+                      uint32_t* d_n_seeds, int32_t* d_status, cudaStream_t s);
+
 // Everything of tt_trigger_slice.  last == nullptr: L1 by l1_tile_kernel.  last != nullptr: the last merge level has
 // written the in-tile L1 flags (fused call); the tile edges are finished here.
 static int trigger_run(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
@@ -1117,6 +1121,15 @@ static int trigger_run(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg
     prof_mark(s, "trig.l1_compact");
     TT_K(l1_compact_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1,
                                                          g->dev.n_pmt, g->dev.ppt, d_status);
+    return trigger_l2(plan, n, d_seg_offsets, n_seg, g, p, d_flags, d_seeds, seed_cap, d_n_seeds, d_status, s);
+}
+
+// L2 (rows, clique, wide) and the ordered seed list over the L1 list plan.l1[*plan.m_total].  `n` bounds the `idx`
+// fields of the list (the sorted hit array, or the list itself in tt_l2_merged); flags / seeds are indexed by them.
+static int trigger_l2(const TriggerPlan& plan, uint32_t n, const uint32_t* d_seg_offsets, uint32_t n_seg,
+                      const tt_geometry* g, const tt_params* p, uint8_t* d_flags, uint32_t* d_seeds, uint32_t seed_cap,
+                      uint32_t* d_n_seeds, int32_t* d_status, cudaStream_t s) {
+    const uint32_t sms = (uint32_t)sm_count();
     prof_mark(s, "trig.l2_rows");
     TT_CUDA_OK(cudaMemsetAsync(plan.slow_cnt, 0, 4 * sizeof(uint32_t), s));
     const uint32_t nt2 = g->dev.n_tower * g->dev.n_tower;
@@ -1226,4 +1239,297 @@ extern "C" int tt_sort_trigger_slice(const tt_hit* d_in, tt_hit* d_out, uint32_t
     if (rc != TT_OK) return rc;
     return trigger_run(d_out, n, d_seg_offsets, n_seg, g, p, d_flags, d_seeds, seed_cap, d_n_seeds, d_ws_trig, d_status, s,
                        &last);
+}
+
+// ------------------------------------------------------------------------------------------------
+// NEXT-4: the trigger of a multi-tower detector sharded BY TOWER over several GPUs, with ONE exchange (PAPER.md:81,
+// sect. 5: "each TGPU finds the trigger seeds of its tower and sends them to a TCPU ... gets candidate times back";
+// SURVEY.md 8(e)(ii)).  L1 is local to a floor, hence to a tower: every rank sorts and L1-tags the hits of its own
+// towers (tt_sort_l1_slice), exports its L1 hits as 16-byte records (tt_l1_export), the ranks all-gather them
+// (~2 % of the hits), merge the lists in time (tt_sort_slice: the record starts with the time, like a hit), and every
+// rank evaluates the inter-tower L2 on the merged list (tt_l2_merged: the same kernels as tt_trigger_slice), takes the
+// bits of its own hits (tt_l2_apply) and tags its hits inside the global event windows (tt_tag_windows).  The result
+// is, hit for hit, what one GPU computes on the whole detector.
+// ------------------------------------------------------------------------------------------------
+namespace tt {
+
+struct L1Hit {  // = tt_l1hit
+    int64_t t;
+    uint32_t idx;
+    uint32_t ps;  // pmt_id | src << 16
+};
+
+__global__ void __launch_bounds__(kL1Threads) l1_export_kernel(const uint4* __restrict__ hits, uint32_t n,
+                                                               const uint8_t* __restrict__ flags,
+                                                               const uint32_t* __restrict__ tile_off, uint32_t src,
+                                                               L1Hit* __restrict__ out, uint32_t cap) {
+    __shared__ uint32_t sm[33];
+    const uint32_t i0 = blockIdx.x * (uint32_t)kL1Tile + threadIdx.x * kL1Per;
+    uint32_t mask = 0;
+    for (uint32_t k = 0; k < (uint32_t)kL1Per && i0 + k < n; ++k)
+        if (flags[i0 + k] & TT_L1) mask |= 1u << k;
+    uint32_t total;
+    uint32_t r = tile_off[blockIdx.x] + block_exclusive_scan(__popc(mask), sm, &total);
+    while (mask) {
+        const uint32_t k = __ffs(mask) - 1;
+        mask &= mask - 1;
+        const uint32_t i = i0 + k;
+        const uint4 v = __ldg(hits + i);
+        L1Hit h;
+        h.t = hit_time(v);
+        h.idx = i;
+        h.ps = (v.z & 0xFFFFu) | (src << 16);
+        if (r < cap) out[r] = h;
+        ++r;
+    }
+}
+
+__global__ void __launch_bounds__(256) l1_export_finish_kernel(const uint32_t* __restrict__ m_total, uint32_t cap,
+                                                               uint32_t* __restrict__ n_out, int32_t* __restrict__ status) {
+    if (threadIdx.x == 0 && blockIdx.x == 0) {
+        *n_out = *m_total;
+        if (*m_total > cap) atomicOr(status, TT_S_L1_OVERFLOW);
+    }
+}
+
+__global__ void __launch_bounds__(256) l1hit_to_rec_kernel(const L1Hit* __restrict__ in, uint32_t m, uint32_t n_pmt,
+                                                           uint32_t ppt, L1Rec* __restrict__ out,
+                                                           uint32_t* __restrict__ m_total, int32_t* __restrict__ status) {
+    const uint32_t x = blockIdx.x * blockDim.x + threadIdx.x;
+    if (x == 0) *m_total = m;
+    bool bad = false;
+    if (x < m) {
+        const L1Hit h = in[x];
+        L1Rec rec;
+        rec.t = h.t;
+        rec.idx = x;  // flags and seeds of tt_l2_merged are indexed by the position in the merged list
+        const uint32_t pmt = h.ps & 0xFFFFu;
+        if (pmt >= n_pmt) { rec.tp = kBadTp; bad = true; }
+        else { const uint32_t tw = pmt / ppt; rec.tp = (tw << 16) | (pmt - tw * ppt); }
+        out[x] = rec;
+    }
+    if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(status, TT_S_BAD_PMT);
+}
+
+__global__ void __launch_bounds__(kSeedThreads) l2_apply_count_kernel(const L1Hit* __restrict__ l1, const uint8_t* __restrict__ bits,
+                                                                      uint32_t m, uint32_t src, uint32_t* __restrict__ cnt) {
+    const uint32_t per = (m + gridDim.x - 1) / gridDim.x;
+    const uint64_t a = (uint64_t)blockIdx.x * per;
+    const uint32_t c0 = a < m ? (uint32_t)a : m, c1 = a + per < m ? (uint32_t)(a + per) : m;
+    uint32_t c = 0;
+    for (uint32_t x = c0 + threadIdx.x; x < c1; x += kSeedThreads)
+        c += ((l1[x].ps >> 16) == src && (bits[x] & TT_L2)) ? 1u : 0u;
+    __shared__ uint32_t sm[33];
+    uint32_t total;
+    block_exclusive_scan(c, sm, &total);
+    if (threadIdx.x == 0) cnt[blockIdx.x] = total;
+}
+
+__global__ void __launch_bounds__(kSeedThreads) l2_apply_write_kernel(const L1Hit* __restrict__ l1, const uint8_t* __restrict__ bits,
+                                                                      uint32_t m, uint32_t src, const uint32_t* __restrict__ off,
+                                                                      uint8_t* __restrict__ flags, uint32_t n,
+                                                                      uint32_t* __restrict__ seeds, uint32_t cap) {
+    __shared__ uint32_t sm[33];
+    const uint32_t per = (m + gridDim.x - 1) / gridDim.x;
+    const uint64_t a = (uint64_t)blockIdx.x * per;
+    const uint32_t c0 = a < m ? (uint32_t)a : m, c1 = a + per < m ? (uint32_t)(a + per) : m;
+    uint32_t run = off[blockIdx.x];
+    for (uint32_t base = c0; base < c1; base += kSeedThreads) {
+        const uint32_t x = base + threadIdx.x;
+        bool is = false;
+        uint32_t idx = 0;
+        if (x < c1) {
+            const L1Hit h = l1[x];
+            if ((h.ps >> 16) == src && h.idx < n) {
+                const uint32_t b = bits[x] & (uint32_t)(TT_L2STAR | TT_L2);
+                idx = h.idx;
+                flags[idx] = (uint8_t)((flags[idx] & ~(uint32_t)(TT_L2STAR | TT_L2)) | b);  // one record per hit: no race
+                is = (b & TT_L2) != 0;
+            }
+        }
+        uint32_t total;
+        const uint32_t r = block_exclusive_scan(is ? 1u : 0u, sm, &total);
+        if (is && run + r < cap) seeds[run + r] = idx;
+        run += total;
+    }
+}
+
+// INEVT for the hits of a sorted slice that lie inside one of the (ascending, disjoint) event windows
+// [t_first - H, t_last + H], t_first = t_start + H and t_last = t_end - H (exact for any int64: unsigned differences)
+__global__ void __launch_bounds__(256) tag_windows_kernel(const uint4* __restrict__ hits, uint32_t n,
+                                                          const tt_event* __restrict__ events,
+                                                          const uint32_t* __restrict__ n_events_ptr, uint32_t event_cap,
+                                                          uint64_t H, uint8_t* __restrict__ flags) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t ne = min(*n_events_ptr, event_cap);
+    if (i >= n || ne == 0) return;
+    const int64_t t = hit_time(__ldg(hits + i));
+    uint32_t a = 0, b = ne;  // first event with t <= t_last + H
+    while (a < b) {
+        const uint32_t mid = a + ((b - a) >> 1);
+        const int64_t t_last = (int64_t)((uint64_t)events[mid].t_end - H);
+        if (t <= t_last || udiff(t, t_last) <= H) b = mid; else a = mid + 1;
+    }
+    if (a < ne) {
+        const int64_t t_first = (int64_t)((uint64_t)events[a].t_start + H);
+        if (t >= t_first || udiff(t_first, t) <= H) flags[i] |= (uint8_t)TT_INEVT;
+    }
+}
+
+struct ExportPlan {
+    uint32_t *blk_cnt, *scan_scratch, *m_total;
+    uint32_t nblk;
+};
+static void export_plan(Arena& a, uint32_t n, ExportPlan& p) {
+    p.nblk = div_up(n, kL1Tile);
+    p.blk_cnt = a.take<uint32_t>(p.nblk + 1);
+    p.scan_scratch = a.take<uint32_t>(scan_ws_count(p.nblk + 1));
+    p.m_total = a.take<uint32_t>(1);
+}
+
+}  // namespace tt
+
+extern "C" int tt_sort_l1_slice(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_t n,
+                                const uint32_t* d_seg_offsets, const uint32_t* h_seg_offsets, uint32_t n_seg,
+                                const uint32_t* d_run_offsets, const uint32_t* h_run_offsets, uint32_t n_runs,
+                                const tt_params* p, uint8_t* d_flags, void* d_ws, size_t* ws_bytes, int32_t* d_status,
+                                void* stream) {
+    if (!ws_bytes || !p || p->lc_window_ps < 0 || !h_run_offsets || n_runs < 1) return TT_E_INVAL;
+    size_t need = 0;
+    int rc = tt_sort_slice(nullptr, nullptr, nullptr, n, nullptr, h_seg_offsets, n_seg, d_run_offsets ? d_run_offsets : h_run_offsets,
+                           h_run_offsets, n_runs, nullptr, &need, nullptr, nullptr);
+    if (rc != TT_OK) return rc;
+    if (!d_ws) {
+        *ws_bytes = need;
+        return TT_OK;
+    }
+    if (*ws_bytes < need) return TT_E_WORKSPACE;
+    if (n == 0) return TT_OK;
+    if (!d_in || !d_out || !d_seg_offsets || !d_run_offsets || !d_flags || !d_status || d_in == d_out) return TT_E_INVAL;
+    if (((uintptr_t)d_ws & 255) || ((uintptr_t)d_in & 15) || ((uintptr_t)d_out & 15)) return TT_E_INVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    FuseL1 fz;
+    fz.flags = d_flags;
+    fz.lc = (uint64_t)p->lc_window_ps;
+    fz.q_thresh = p->q_thresh;
+    MergeLast last;
+    last.tiles = 0;
+    rc = merge_sort_runs(d_in, d_out, d_perm, n, d_seg_offsets, h_seg_offsets, n_seg, d_run_offsets, h_run_offsets, n_runs,
+                         d_ws, d_status, s, &fz, &last);
+    if (rc != TT_OK) return rc;
+    prof_mark(s, "trig.l1_edges");
+    if (last.tiles)
+        TT_K(l1_boundary_kernel)<<<div_up(last.tiles, kBndWarps), kBndWarps * 32, 0, s>>>(
+            last.lv, last.tiles, (const uint4*)d_out, (uint64_t)p->lc_window_ps, p->q_thresh, d_flags);
+    prof_end(s);
+    TT_LAUNCH_OK();
+    return TT_OK;
+}
+
+extern "C" int tt_l1_export(const tt_hit* d_sorted, uint32_t n, const uint8_t* d_flags, uint32_t src, tt_l1hit* d_l1,
+                            uint32_t l1_cap, uint32_t* d_n_l1, void* d_ws, size_t* ws_bytes, int32_t* d_status,
+                            void* stream) {
+    if (!ws_bytes || src > 0xFFFFu || n >= 0xFFF00000u) return TT_E_INVAL;
+    Arena sizing(nullptr);
+    ExportPlan plan;
+    export_plan(sizing, n, plan);
+    if (!d_ws) {
+        *ws_bytes = sizing.off;
+        return TT_OK;
+    }
+    if (*ws_bytes < sizing.off) return TT_E_WORKSPACE;
+    if (!d_n_l1 || !d_status || (n && (!d_sorted || !d_flags)) || (l1_cap && !d_l1) || ((uintptr_t)d_ws & 255)) return TT_E_INVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n == 0) {
+        TT_CUDA_OK(cudaMemsetAsync(d_n_l1, 0, sizeof(uint32_t), s));
+        return TT_OK;
+    }
+    Arena a(d_ws);
+    export_plan(a, n, plan);
+    prof_mark(s, "towers.l1_export");
+    TT_K(l1_count_kernel)<<<plan.nblk, kL1Threads, 0, s>>>(d_flags, n, plan.blk_cnt);
+    int rc = exclusive_scan_u32(plan.blk_cnt, plan.blk_cnt, plan.nblk, plan.scan_scratch, plan.m_total, s);
+    if (rc != TT_OK) return rc;
+    TT_K(l1_export_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, src,
+                                                         reinterpret_cast<L1Hit*>(d_l1), l1_cap);
+    TT_K(l1_export_finish_kernel)<<<1, 32, 0, s>>>(plan.m_total, l1_cap, d_n_l1, d_status);
+    prof_end(s);
+    TT_LAUNCH_OK();
+    return TT_OK;
+}
+
+extern "C" int tt_l2_merged(const tt_l1hit* d_l1, uint32_t m, const tt_geometry* g, const tt_params* p, uint8_t* d_bits,
+                            uint32_t* d_seeds, uint32_t seed_cap, uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes,
+                            int32_t* d_status, void* stream) {
+    if (!ws_bytes) return TT_E_INVAL;
+    const uint32_t seg1[2] = {0, m};
+    int rc = trigger_args_ok(m, seg1, 1, g, p);
+    if (rc != TT_OK) return rc;
+    Arena sizing(nullptr);
+    TriggerPlan plan;
+    trigger_plan(sizing, m, plan);
+    if (!d_ws) {
+        *ws_bytes = sizing.off;
+        return TT_OK;
+    }
+    if (*ws_bytes < sizing.off) return TT_E_WORKSPACE;
+    if (!d_n_seeds || !d_status || (!d_seeds && seed_cap) || (m && (!d_l1 || !d_bits)) || ((uintptr_t)d_ws & 255)) return TT_E_INVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (m == 0) {
+        TT_CUDA_OK(cudaMemsetAsync(d_n_seeds, 0, sizeof(uint32_t), s));
+        return TT_OK;
+    }
+    Arena a(d_ws);
+    trigger_plan(a, m, plan);
+    rc = once_per_device(kSlotTrigger, trigger_attrs);
+    if (rc != TT_OK) return rc;
+    prof_mark(s, "towers.l2_prepare");
+    TT_CUDA_OK(cudaMemsetAsync(d_bits, 0, m, s));
+    TT_K(l1hit_to_rec_kernel)<<<div_up(m, 256), 256, 0, s>>>(reinterpret_cast<const L1Hit*>(d_l1), m, g->dev.n_pmt, g->dev.ppt,
+                                                            plan.l1, plan.m_total, d_status);
+    return trigger_l2(plan, m, nullptr, 1, g, p, d_bits, d_seeds, seed_cap, d_n_seeds, d_status, s);
+}
+
+extern "C" int tt_l2_apply(const tt_l1hit* d_l1, const uint8_t* d_bits, uint32_t m, uint32_t src, uint8_t* d_flags, uint32_t n,
+                           uint32_t* d_seeds, uint32_t seed_cap, uint32_t* d_n_seeds, void* d_ws, size_t* ws_bytes,
+                           int32_t* d_status, void* stream) {
+    if (!ws_bytes || src > 0xFFFFu) return TT_E_INVAL;
+    Arena sizing(nullptr);
+    (void)sizing.take<uint32_t>(kSeedBlocks);
+    if (!d_ws) {
+        *ws_bytes = sizing.off;
+        return TT_OK;
+    }
+    if (*ws_bytes < sizing.off) return TT_E_WORKSPACE;
+    if (!d_n_seeds || !d_status || (!d_seeds && seed_cap) || (m && (!d_l1 || !d_bits || !d_flags)) || ((uintptr_t)d_ws & 255))
+        return TT_E_INVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (m == 0) {
+        TT_CUDA_OK(cudaMemsetAsync(d_n_seeds, 0, sizeof(uint32_t), s));
+        return TT_OK;
+    }
+    Arena a(d_ws);
+    uint32_t* cnt = a.take<uint32_t>(kSeedBlocks);
+    prof_mark(s, "towers.l2_apply");
+    TT_K(l2_apply_count_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(reinterpret_cast<const L1Hit*>(d_l1), d_bits, m, src, cnt);
+    TT_K(count_scan_kernel)<<<1, 1024, 0, s>>>(cnt, kSeedBlocks, d_n_seeds, seed_cap, TT_S_SEED_OVERFLOW, d_status);
+    TT_K(l2_apply_write_kernel)<<<kSeedBlocks, kSeedThreads, 0, s>>>(reinterpret_cast<const L1Hit*>(d_l1), d_bits, m, src, cnt,
+                                                                   d_flags, n, d_seeds, seed_cap);
+    prof_end(s);
+    TT_LAUNCH_OK();
+    return TT_OK;
+}
+
+extern "C" int tt_tag_windows(const tt_hit* d_sorted, uint32_t n, const tt_event* d_events, const uint32_t* d_n_events,
+                              uint32_t event_cap, const tt_params* p, uint8_t* d_flags, void* stream) {
+    if (!p || p->event_half_ps < 0 || n >= 0xFFF00000u) return TT_E_INVAL;
+    if (n == 0) return TT_OK;
+    if (!d_sorted || !d_events || !d_n_events || !d_flags) return TT_E_INVAL;
+    cudaStream_t s = (cudaStream_t)stream;
+    prof_mark(s, "towers.tag_windows");
+    TT_K(tag_windows_kernel)<<<div_up(n, 256), 256, 0, s>>>((const uint4*)d_sorted, n, d_events, d_n_events, event_cap,
+                                                           (uint64_t)p->event_half_ps, d_flags);
+    prof_end(s);
+    TT_LAUNCH_OK();
+    return TT_OK;
 }
