@@ -269,6 +269,57 @@ def time_radix(B, run, peak):
             "note": "8-bit LSD passes over the varying key bits + one gather: ~5 passes x (12 B read + 24 B moved)"}
 
 
+def time_tower_shard(B, w, geo, prm, ranks):
+    """NEXT-4: ONE cfg4 slice sharded by tower over `ranks` GPUs with one exchange of L1 hits.  This box has
+    one GPU, so the ranks are EMULATED one after the other (no kernel waits on another rank): what is reported is the
+    per-rank device time of the two phases and the bytes a rank would all-gather -- not a multi-GPU measurement."""
+    import torch
+
+    from paper_1411_3968_b200 import sharding
+
+    g = w.geometry
+    parts = sharding.split_runs_by_tower(w.run_offsets, g.pmts_per_tower, g.n_tower, ranks)
+    d_parts = [(B.hits_to_device(np.ascontiguousarray(w.hits[a:b])), B.Offsets(ro)) for a, b, ro in parts]
+
+    def ev_pair():
+        return torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+
+    def phase1():
+        out, tms = [], []
+        for r, (d_h, ro) in enumerate(d_parts):
+            e0, e1 = ev_pair()
+            e0.record()
+            out.append(sharding.tower_local(B, r, d_h, ro, prm))  # ends with the read-back of the rank's L1 count
+            e1.record()
+            torch.cuda.synchronize()
+            tms.append(e0.elapsed_time(e1))
+        return out, tms
+
+    phase1()  # warm-up (allocator, plans)
+    states, t_local = phase1()
+    gathered = torch.cat([s["l1"] for s in states], dim=0)
+    offs = [0]
+    for s in states:
+        offs.append(offs[-1] + int(s["l1"].shape[0]))
+    t_global, seeds = [], 0
+    for rep in range(3):
+        for s in states[:2]:  # the global phase does the same work on every rank: two of them are timed
+            e0, e1 = ev_pair()
+            e0.record()
+            res = sharding.tower_global(B, s, gathered, offs, geo, prm, download=False)
+            e1.record()
+            torch.cuda.synchronize()
+            if rep:
+                t_global.append(e0.elapsed_time(e1))
+            seeds = int(res["d_counts"].cpu().numpy().view(np.uint32)[0])
+    return {"ranks_emulated": ranks, "hits": w.n, "l1_records_total": int(gathered.shape[0]),
+            "all_gather_bytes_per_rank": int(16 * gathered.shape[0]),
+            "local_phase_ms_max_over_ranks": max(t_local), "global_phase_ms": max(t_global), "global_seeds": seeds,
+            "note": "ranks emulated sequentially on one GPU, device-resident input and output (CUDA events; buffer "
+                    "allocation inside); a step of the sharded path = local phase + all-gather + global phase; "
+                    "tests/test_gpu_towers.py checks the result against the oracle on the whole detector"}
+
+
 def time_prepare(B, peak):
     """tt_prepare_slice (NEXT-3) on the raw stream of a cfg2-shaped burst: five 200 ms sub-slices at
     half the duration (15 M raw hits, 28 B each on average) -> PMT-major 16-byte records + run offsets."""
@@ -647,6 +698,10 @@ def run_ours(args):
     extra = None
     if rank == 0 and world == 1 and not args.no_extra:
         extra = {"configs": {}}
+        if w.geometry.n_tower >= 8:
+            n_seeds_step = n_seeds
+            extra["tower_shard"] = time_tower_shard(B, w, geo, prm, 8)
+            assert extra["tower_shard"]["global_seeds"] == n_seeds_step, "by-tower path disagrees with the single-GPU path"
         del run
         torch.cuda.empty_cache()
         for c2 in [c for c in (0, 1, 2, 3, 4) if c != args.config]:

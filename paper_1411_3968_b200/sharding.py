@@ -93,10 +93,10 @@ def tower_local(B, rank: int, hits, run_offsets, params):
     records.  Returns the state `tower_global` continues from."""
     import numpy as np
 
-    n = len(hits)
+    d_in = hits if isinstance(hits, torch.Tensor) else B.hits_to_device(hits)  # (n, 2) int64 on the device, or numpy hits
+    n = int(d_in.shape[0])
     seg = B.Offsets(np.array([0, n], dtype=np.uint32))
-    runs = B.Offsets(run_offsets)
-    d_in = B.hits_to_device(hits)
+    runs = run_offsets if isinstance(run_offsets, B.Offsets) else B.Offsets(run_offsets)
     d_out = torch.empty_like(d_in)
     d_flags = torch.full((max(n, 1),), 0xEE, dtype=torch.uint8, device="cuda")
     d_st = torch.zeros(1, dtype=torch.int32, device="cuda")
@@ -108,9 +108,10 @@ def tower_local(B, rank: int, hits, run_offsets, params):
     return dict(rank=rank, n=n, d_sorted=d_out, d_flags=d_flags, d_status=d_st, l1=d_l1[:m].contiguous())
 
 
-def tower_global(B, state, gathered: torch.Tensor, offsets: list[int], geo, params):
+def tower_global(B, state, gathered: torch.Tensor, offsets: list[int], geo, params, download: bool = True):
     """Phase 2: merge the gathered L1 records in time, inter-tower L2 on the merged list, global event windows, then
-    this rank's flag bits, seeds and INEVT tags.  Returns numpy arrays: flags, seeds (local indices), events."""
+    this rank's flag bits, seeds and INEVT tags.  Returns numpy arrays: flags, seeds (local indices), events
+    (download=False: leaves everything on the device and returns the device tensors)."""
     import numpy as np
 
     m = int(gathered.shape[0])
@@ -130,6 +131,8 @@ def tower_global(B, state, gathered: torch.Tensor, offsets: list[int], geo, para
     d_seeds = torch.zeros(max(n, 1), dtype=torch.int32, device="cuda")
     B.tt_l2_apply(d_l1m, d_bits, state["rank"], state["d_flags"], n, d_seeds, d_cnt[2:3], d_st)
     B.tt_tag_windows(state["d_sorted"], d_ev, d_cnt[1:2], params, state["d_flags"])
+    if not download:
+        return dict(d_flags=state["d_flags"], d_seeds=d_seeds, d_events=d_ev, d_counts=d_cnt)
     torch.cuda.synchronize()
     cnt = d_cnt.cpu().numpy().view(np.uint32)
     return dict(sorted=B.hits_to_host(state["d_sorted"]), flags=state["d_flags"].cpu().numpy()[:n].copy(),
