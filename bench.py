@@ -269,6 +269,55 @@ def time_radix(B, run, peak):
             "note": "8-bit LSD passes over the varying key bits + one gather: ~5 passes x (12 B read + 24 B moved)"}
 
 
+def time_streams(B, run, steps):
+    """BASELINE.json configs[3]: "64 independent slices processed concurrently on one GPU through CUDA streams".  The
+    same work as run.step(), but one call chain per segment (n_seg = 1) on its own stream, against the single
+    segmented call the timed step uses (compare the two).  Direct launches both ways."""
+    import torch
+
+    w = run.w
+    seg = np.asarray(w.seg_offsets, dtype=np.int64)
+    ro = np.asarray(w.run_offsets, dtype=np.int64)
+    n_seg = len(seg) - 1
+    streams = [torch.cuda.Stream() for _ in range(n_seg)]
+    parts = []
+    for s in range(n_seg):
+        a, b = int(seg[s]), int(seg[s + 1])
+        r0, r1 = int(np.searchsorted(ro, a, side="left")), int(np.searchsorted(ro, b, side="left"))
+        cap = max((b - a) // 4, 1024)
+        parts.append(dict(a=a, b=b, seg=B.Offsets(np.array([0, b - a], dtype=np.uint32)),
+                          runs=B.Offsets((ro[r0:r1 + 1] - a).astype(np.uint32)),
+                          seeds=torch.zeros(cap, dtype=torch.int32, device="cuda"),
+                          ev=torch.zeros((cap, 4), dtype=torch.int64, device="cuda"),
+                          cnt=torch.zeros(4, dtype=torch.int32, device="cuda"), ws={}))
+
+    def step():
+        start = torch.cuda.Event()
+        start.record()
+        for st, pt in zip(streams, parts):
+            st.wait_event(start)
+            with torch.cuda.stream(st):
+                a, b, c, ws = pt["a"], pt["b"], pt["cnt"], pt["ws"]
+                c.zero_()
+                ws["f"] = B.tt_sort_trigger_slice(run.d_in[a:b], run.d_out[a:b], None, pt["seg"], pt["runs"], run.geo, run.prm,
+                                                  run.d_flags[a:b], pt["seeds"], c[0:1], c[2:3], ws.get("f"))
+                ws["e"] = B.tt_extract_events(run.d_out[a:b], pt["seg"], pt["seeds"], c[0:1], run.prm, pt["ev"], c[1:2],
+                                              run.d_flags[a:b], None, None, c[2:3], ws.get("e"))
+        for st in streams:
+            torch.cuda.current_stream().wait_stream(st)
+
+    for _ in range(2):
+        step()
+    torch.cuda.synchronize()
+    ns = sum(int(pt["cnt"][0].item()) for pt in parts)
+    ms_streams = _cuda_time(step, max(2, min(steps, 5)))
+    B.prof_enable(False)
+    ms_one = _cuda_time(run.step, max(2, min(steps, 5)))
+    return {"segments": n_seg, "ms_per_step_one_stream_per_segment": ms_streams, "ms_per_step_one_segmented_call": ms_one,
+            "n_seeds_streams": ns,
+            "note": "direct launches both ways (no CUDA graph); the default timed step is the segmented call replayed as a graph"}
+
+
 def time_tower_shard(B, w, geo, prm, ranks):
     """NEXT-4: ONE cfg4 slice sharded by tower over `ranks` GPUs with one exchange of L1 hits.  This box has
     one GPU, so the ranks are EMULATED one after the other (no kernel waits on another rank): what is reported is the
@@ -713,6 +762,9 @@ def run_ours(args):
                 "pipeline_frac": ALG_BYTES_PIPELINE * r2.n / (m2["ms_step"] * 1e-3) / 1e9 / peak,
                 "stages": {k: v["frac"] for k, v in stage_fracs(m2["per_stage"], r2.n, peak).items()},
                 "n_seeds": m2["n_seeds"], "n_events": m2["n_events"], "status": m2["status"]}
+            if c2 == 3:
+                extra["cfg3_streams_vs_segmented"] = time_streams(B, r2, args.steps)
+                assert extra["cfg3_streams_vs_segmented"]["n_seeds_streams"] == m2["n_seeds"], "per-stream path disagrees"
             if c2 == 1:
                 extra["radix_unsorted_input"] = time_radix(B, r2, peak)
             if c2 == 2:

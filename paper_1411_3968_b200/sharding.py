@@ -73,6 +73,10 @@ def all_gather_records(rec: torch.Tensor) -> tuple[torch.Tensor, list[int]]:
     if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
         return rec, [0, int(rec.shape[0])]
     world = dist.get_world_size()
+    dev = rec.device
+    if rec.is_cuda and dist.get_backend() == "gloo":  # gloo moves host memory: stage through the host and come back
+        cat, offs = all_gather_records(rec.cpu())
+        return cat.to(dev), offs
     cnt = torch.tensor([rec.shape[0]], dtype=torch.int64, device=rec.device)
     cnts = [torch.zeros_like(cnt) for _ in range(world)]
     dist.all_gather(cnts, cnt)

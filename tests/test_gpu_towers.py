@@ -96,3 +96,66 @@ def test_l1_export_overflow_and_empty(B, oracle_lib):
     torch.cuda.synchronize()
     assert int(d_m.item()) == len(want) and int(d_st.item()) == B.TT_S_L1_OVERFLOW
     assert (d_l1.cpu().numpy().reshape(-1).view(B.L1HIT_DTYPE)["idx"] == want[:3]).all()
+
+
+def _tower_worker(rank: int, world: int, port: int, out):
+    import os
+
+    import torch.distributed as dist
+
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)  # NCCL refuses two ranks on one GPU; the exchange is the same code
+    try:
+        from paper_1411_3968_b200 import binding as Bn
+
+        torch.cuda.set_device(0)
+        Bn.load()
+        w = W.make_config(4, time_scale=0.002)  # every rank sees the same slice and takes its towers
+        p, g = w.params, w.geometry
+        geo = Bn.Geometry(g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks)
+        prm = Bn.make_params(p.q_thresh, p.lc_window_ps, p.l2_window_ps, p.l2_multiplicity, p.l2_mode, p.event_half_ps)
+        a, b, ro = sharding.split_runs_by_tower(w.run_offsets, g.pmts_per_tower, g.n_tower, world)[rank]
+        st = sharding.tower_local(Bn, rank, np.ascontiguousarray(w.hits[a:b]), ro, prm)
+        gathered, offs = sharding.all_gather_records(st["l1"])
+        res = sharding.tower_global(Bn, st, gathered, offs, geo, prm)
+        out.put((rank, res["flags"].tobytes(), res["seeds"].tobytes(), res["events"].tobytes(), res["n_global_seeds"], res["status"]))
+    finally:
+        dist.destroy_process_group()
+
+
+def test_by_tower_two_processes(B, oracle_lib):
+    """The real multi-process flow: two ranks (processes), each computing on the GPU, exchanging their L1 records through
+    torch.distributed (gloo here: both share the box's one GPU), against the oracle on the whole detector."""
+    import socket
+
+    import torch.multiprocessing as mp
+
+    world = 2
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    out = ctx.Queue()
+    procs = [ctx.Process(target=_tower_worker, args=(r, world, port, out)) for r in range(world)]
+    for pr in procs:
+        pr.start()
+    got = {}
+    for _ in range(world):
+        r = out.get(timeout=600)
+        got[r[0]] = r
+    for pr in procs:
+        pr.join(timeout=120)
+        assert pr.exitcode == 0
+    w = W.make_config(4, time_scale=0.002)
+    g = w.geometry
+    o = oracle_chain(w.hits, w.seg_offsets, g, w.params)
+    tower = o["sorted"]["pmt_id"].astype(np.int64) // g.pmts_per_tower
+    for r, (lo, hi) in enumerate(sharding.tower_ranges(g.n_tower, world)):
+        mine = (tower >= lo) & (tower < hi)
+        _, fl, sd, ev, ngs, st = got[r]
+        assert st == 0 and ngs == len(o["seeds"])
+        assert fl == o["flags"][mine].tobytes(), f"rank {r}: flags"
+        assert sd == np.nonzero(o["flags"][mine] & 16)[0].astype(np.uint32).tobytes(), f"rank {r}: seeds"
+        evs = np.frombuffer(ev, dtype=B.EVENT_DTYPE)
+        assert len(evs) == len(o["events"]) and (evs["t_start"] == o["events"]["t_start"]).all() and (evs["t_end"] == o["events"]["t_end"]).all()
