@@ -342,20 +342,29 @@ __global__ void __launch_bounds__(kL1Threads) l1_compact_kernel(const uint4* __r
                 if (flags[i0 + k] & TT_L1) mask |= 1u << k;
         }
     }
+    // the block's L1 hits as a dense list of tile positions in shared memory (a tile holds ~2 % L1 hits: most threads
+    // have none, a few have one), then one thread per list entry: the record gathers are all in flight at once and
+    // the 16-byte list records leave coalesced
+    __shared__ uint16_t s_pos[kL1Tile];
     uint32_t total;
-    uint32_t r = tile_off[blockIdx.x] + block_exclusive_scan(__popc(mask), sm, &total);
-    bool bad = false;
+    uint32_t r = block_exclusive_scan(__popc(mask), sm, &total);
     while (mask) {
         const uint32_t k = __ffs(mask) - 1;
         mask &= mask - 1;
-        const uint32_t i = i0 + k;
+        s_pos[r++] = (uint16_t)(threadIdx.x * kL1Per + k);
+    }
+    __syncthreads();
+    const uint32_t base = tile_off[blockIdx.x], tb = blockIdx.x * (uint32_t)kL1Tile;
+    bool bad = false;
+    for (uint32_t q = threadIdx.x; q < total; q += kL1Threads) {
+        const uint32_t i = tb + s_pos[q];
         const HitView h = unpack(__ldg(hits + i));
         L1Rec rec;
         rec.t = h.t;
         rec.idx = i;
         if (h.pmt >= n_pmt) { rec.tp = kBadTp; bad = true; }
         else { const uint32_t tw = h.pmt / ppt; rec.tp = (tw << 16) | (h.pmt - tw * ppt); }
-        l1[r++] = rec;
+        l1[base + q] = rec;
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(status, TT_S_BAD_PMT);
 }
