@@ -1,0 +1,86 @@
+"""Seeded random inputs through the whole chain, fused and three-call, against the oracle: segment counts, run counts
+(one to several hundred per segment, two merge levels included), empty runs and segments, time distributions (uniform,
+clustered, heavy ties, wide spans), windows, multiplicities and modes drawn at random -- the shapes between the five
+configs and the hand-written edge cases."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1411_3968_b200 import workload as W
+from util import oracle_chain, single_tower_geo
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_1411_3968_b200 import binding
+
+    binding.load()
+    return binding
+
+
+def _case(seed):
+    rng = np.random.default_rng(1000 + seed)
+    P = int(rng.choice([1, 2, 7, 32, 84, 128]))
+    n_seg = int(rng.integers(1, 6))
+    kind = rng.choice(["uniform", "clustered", "ties", "wide", "dense"])
+    span = {"uniform": 10**9, "clustered": 10**9, "ties": 4000, "wide": 2**45, "dense": 3 * 10**6}[kind]
+    parts, runs, seg = [], [0], [0]
+    for s in range(n_seg):
+        n_runs = int(rng.choice([1, 3, 84, 300, 700])) if rng.random() < 0.8 else 0
+        n_s = int(rng.integers(0, 8_000 if kind in ("ties", "dense") else 30_000)) if n_runs else 0  # (dense kinds: the oracle is O(n^2))
+        t0 = int(rng.integers(-2**40, 2**40))
+        t = t0 + rng.integers(0, span, size=n_s)
+        if kind == "clustered" and n_s:
+            c = t0 + rng.integers(0, span, size=8)
+            t = c[rng.integers(0, 8, size=n_s)] + rng.integers(0, 200_000, size=n_s)
+        which = rng.integers(0, max(n_runs, 1), size=n_s)
+        if n_runs and rng.random() < 0.5:
+            which = np.minimum(which, rng.integers(0, n_runs))  # leaves the upper runs empty
+        h = np.zeros(n_s, dtype=W.HIT_DTYPE)
+        h["t_ps"] = t
+        h["pmt_id"] = rng.integers(0, P, size=n_s)
+        h["floor"] = h["pmt_id"] // 3
+        h["charge"] = rng.integers(1, 400, size=n_s)
+        h["pad"] = rng.integers(0, 65536, size=n_s)
+        o = np.lexsort((t, which))  # run-major, time-ordered inside a run
+        parts.append(h[o])
+        cnt = np.bincount(which, minlength=n_runs) if n_runs else np.zeros(0, dtype=np.int64)
+        for c in cnt:
+            runs.append(runs[-1] + int(c))
+        seg.append(seg[-1] + n_s)
+    hits = np.concatenate(parts) if parts else np.zeros(0, dtype=W.HIT_DTYPE)
+    if len(runs) == 1:
+        runs.append(0)  # at least one (empty) run
+    tab = rng.integers(-1, 400_000, size=(P, P)).astype(np.int32)
+    tab = np.minimum(tab, tab.T)
+    np.fill_diagonal(tab, 20_000)
+    p = W.Params(q_thresh=int(rng.choice([1, 300, 390, 500])), lc_window_ps=int(rng.choice([0, 500, 20_000, 10**6])),
+                 l2_window_ps=int(rng.choice([0, 100_000, 3_000_000])), l2_multiplicity=int(rng.integers(1, 7)),
+                 l2_mode=int(rng.integers(0, 2)), event_half_ps=int(rng.choice([0, 1000, 3_000_000])))
+    if kind in ("ties", "dense") or p.lc_window_ps >= 10**6:
+        p.l2_mode = 1  # dense L1 sets: keep the oracle's clique search out of it
+    return hits, np.asarray(seg, dtype=np.uint32), np.asarray(runs, dtype=np.uint32), single_tower_geo(tab), p
+
+
+@pytest.mark.parametrize("seed", range(36))
+def test_random_chain(seed, B, oracle_lib):
+    hits, seg, runs, g, p = _case(seed)
+    o = oracle_chain(hits, seg, g, p)
+    geo = B.Geometry(g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks)
+    prm = B.make_params(p.q_thresh, p.lc_window_ps, p.l2_window_ps, p.l2_multiplicity, p.l2_mode, p.event_half_ps)
+    for fused in (True, False):
+        r = B.process_slice(hits, seg, runs, geo, prm, fused=fused)
+        assert r.sorted.tobytes() == o["sorted"].tobytes(), (seed, fused)
+        assert (r.perm == o["perm"]).all(), (seed, fused)
+        if r.status & B.TT_S_DENSITY:  # more than 2048 L1 candidates in a window: star bits exact, clique fails open
+            assert ((r.flags & 15) == (o["flags"] & 15)).all(), (seed, fused)
+            continue
+        assert r.status == 0, (seed, fused, r.status)
+        bad = np.nonzero(r.flags != o["flags"])[0]
+        assert len(bad) == 0, (seed, fused, len(bad), bad[:6], r.flags[bad[:6]], o["flags"][bad[:6]])
+        assert r.n_seeds == len(o["seeds"]) and (r.seeds == o["seeds"]).all(), (seed, fused)
+        assert r.n_events == len(o["events"]) and r.events.tobytes() == o["events"].tobytes(), (seed, fused)
+    geo.close()
