@@ -42,9 +42,8 @@ __device__ __forceinline__ uint64_t key_at(const uint4* __restrict__ hits, uint3
 
 // ---- plan step 1: groups.  Segment s owns the runs [lb(roff, seg[s]), lb(roff, seg[s+1])) and is cut into
 // consecutive groups of F runs.  One block; loops over segments with a running carry.
-__global__ void __launch_bounds__(1024) merge_groups_kernel(LevelDev lv, const uint32_t* __restrict__ seg_off,
-                                                            uint32_t n_seg) {
-    __shared__ uint32_t sm[33];
+__device__ __forceinline__ void merge_groups(const LevelDev& lv, const uint32_t* __restrict__ seg_off, uint32_t n_seg,
+                                             uint32_t* sm) {
     uint32_t carry = 0;
     for (uint32_t base = 0; base < n_seg; base += 1024) {
         const uint32_t s = base + threadIdx.x;
@@ -71,22 +70,40 @@ __global__ void __launch_bounds__(1024) merge_groups_kernel(LevelDev lv, const u
 // one warp per group (lanes over the group's runs).
 // run_kmin / run_kmax (nullable): the key range of every run when the runs are the previous level's groups whose hits
 // are not written yet (the previous level's tile kernel emits this level's splits, see emit_next_splits)
-__global__ void __launch_bounds__(1024) merge_setup_kernel(LevelDev lv, const uint4* __restrict__ hits, uint32_t n,
-                                                           const uint64_t* __restrict__ run_kmin,
-                                                           const uint64_t* __restrict__ run_kmax) {
+__global__ void __launch_bounds__(1024) merge_plan_kernel(LevelDev lv, const uint32_t* __restrict__ seg_off, uint32_t n_seg,
+                                                          const uint4* __restrict__ hits, uint32_t n,
+                                                          const uint64_t* __restrict__ run_kmin,
+                                                          const uint64_t* __restrict__ run_kmax) {
     __shared__ uint32_t sm[33];
+    merge_groups(lv, seg_off, n_seg, sm);
+    __syncthreads();  // gfirst[] (global, written by this block) is visible to all its threads
     const uint32_t lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // pass A: per-group ranges (warp per group)
+    // pass A: per-group ranges (warp per group; a lane takes four runs at a time so that their loads overlap)
     for (uint32_t g = warp; g < lv.G; g += 32) {
         const uint32_t r0 = lv.gfirst[g], r1 = lv.gfirst[g + 1];
         uint64_t kmin = ~0ull, kmax = 0;
-        for (uint32_t r = r0 + lane; r < r1; r += 32) {
-            const uint32_t a = lv.roff[r], b = lv.roff[r + 1];
-            lv.run_group[r] = g;
-            if (b > a) {
-                const uint64_t k0 = run_kmin ? run_kmin[r] : key_at(hits, a), k1 = run_kmax ? run_kmax[r] : key_at(hits, b - 1);
-                kmin = k0 < kmin ? k0 : kmin;
-                kmax = k1 > kmax ? k1 : kmax;
+        for (uint32_t rb = r0; rb < r1; rb += 128) {
+            uint32_t a[4], b[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t r = rb + lane + 32u * j;
+                a[j] = 0; b[j] = 0;
+                if (r < r1) { a[j] = lv.roff[r]; b[j] = lv.roff[r + 1]; lv.run_group[r] = g; }
+            }
+            uint64_t k0[4], k1[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const uint32_t r = rb + lane + 32u * j;
+                k0[j] = ~0ull; k1[j] = 0;
+                if (b[j] > a[j]) {
+                    k0[j] = run_kmin ? run_kmin[r] : key_at(hits, a[j]);
+                    k1[j] = run_kmax ? run_kmax[r] : key_at(hits, b[j] - 1);
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                kmin = k0[j] < kmin ? k0[j] : kmin;
+                kmax = k1[j] > kmax ? k1[j] : kmax;
             }
         }
 #pragma unroll
@@ -1055,8 +1072,7 @@ int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_
         uint32_t* pdst = d_perm ? (is_last ? d_perm : w.ptmp[l & 1]) : nullptr;
         if (!planned) {
             prof_mark(s, l == 0 ? "sort.merge_plan0" : "sort.merge_plan1");
-            TT_K(merge_groups_kernel)<<<1, 1024, 0, s>>>(d, d_seg_offsets, n_seg);
-            TT_K(merge_setup_kernel)<<<1, 1024, 0, s>>>(d, src, n, nullptr, nullptr);
+            TT_K(merge_plan_kernel)<<<1, 1024, 0, s>>>(d, d_seg_offsets, n_seg, src, n, nullptr, nullptr);
             TT_CUDA_OK(cudaMemsetAsync(d.tile_base, 0, ((size_t)levels[l].tiles + levels[l].G + 2) * sizeof(uint32_t), s));
             if (levels[l].split_entries) {
                 prof_mark(s, l == 0 ? "sort.merge_partition0" : "sort.merge_partition1");
@@ -1073,8 +1089,7 @@ int merge_sort_runs(const tt_hit* d_in, tt_hit* d_out, uint32_t* d_perm, uint32_
             LevelDev& e = w.dev[l + 1];
             e.roff = d.roff_next;
             prof_mark(s, "sort.merge_plan1");
-            TT_K(merge_groups_kernel)<<<1, 1024, 0, s>>>(e, d_seg_offsets, n_seg);
-            TT_K(merge_setup_kernel)<<<1, 1024, 0, s>>>(e, nullptr, n, d.gT0, d.gKmax);
+            TT_K(merge_plan_kernel)<<<1, 1024, 0, s>>>(e, d_seg_offsets, n_seg, nullptr, n, d.gT0, d.gKmax);
             TT_CUDA_OK(cudaMemsetAsync(e.tile_base, 0, ((size_t)levels[l + 1].tiles + levels[l + 1].G + 2) * sizeof(uint32_t), s));
             TT_K(merge_init_next_kernel)<<<div_up(levels[l + 1].split_entries, 256), 256, 0, s>>>(e, levels[l + 1].split_entries);
             nx = e;
