@@ -261,6 +261,10 @@ CONFIGS = {
             rate="55k", T_ms=200, n_sub=1, n_seg=64, tracks=50, N=5),
     4: dict(name="cfg4 100 KM3NeT-It towers (8400 PMTs), 55 kHz, 1 x 200 ms", kind="km3", nx=10, ny=10,
             rate="55k", T_ms=200, n_sub=1, n_seg=1, tracks=1000, N=5),
+    # not a BASELINE.json config: the "8 towers of KM3NeT-It" of the paper's proposed DAQ (one TGPU per
+    # tower), the workload of the by-tower sharded path; a 4 x 2 grid at the same 90 m pitch
+    5: dict(name="8 KM3NeT-It towers (672 PMTs, PAPER.md:81), 55 kHz, 1 x 200 ms", kind="km3", nx=4, ny=2,
+            rate="55k", T_ms=200, n_sub=1, n_seg=1, tracks=100, N=5),
 }
 
 

@@ -63,6 +63,25 @@ def test_by_tower_equals_whole_detector(world, mode, B, oracle_lib):
     geo.close()
 
 
+def test_eight_towers_one_gpu_per_tower(B, oracle_lib):
+    """The paper's own layout (Fig. 4): 8 towers, one TGPU each -- 8 ranks of one tower (emulated)."""
+    w = W.make_config(5, time_scale=0.05)  # 8 towers, 10 ms: ~370 k hits
+    p, g = w.params, w.geometry
+    assert g.n_tower == 8
+    o = oracle_chain(w.hits, w.seg_offsets, g, p)
+    assert len(o["seeds"]) > 0
+    geo = B.Geometry(g.n_pmt, g.n_tower, g.pmts_per_tower, g.pair_block, g.blocks)
+    prm = B.make_params(p.q_thresh, p.lc_window_ps, p.l2_window_ps, p.l2_multiplicity, p.l2_mode, p.event_half_ps)
+    res = _run_sharded(B, w, 8, prm, geo)
+    tower = o["sorted"]["pmt_id"].astype(np.int64) // g.pmts_per_tower
+    for r in range(8):
+        mine = tower == r
+        assert res[r]["status"] == 0 and (res[r]["flags"] == o["flags"][mine]).all(), r
+        assert (res[r]["seeds"] == np.nonzero(o["flags"][mine] & 16)[0]).all(), r
+        assert (res[r]["events"]["t_start"] == o["events"]["t_start"]).all() and (res[r]["events"]["t_end"] == o["events"]["t_end"]).all()
+    geo.close()
+
+
 def test_by_tower_needs_the_exchange(B, oracle_lib):
     """The exchange is not decoration: a track that crosses towers meets the multiplicity only with the L1 hits of the
     neighbouring towers -- without them (every rank alone) seeds are lost."""
