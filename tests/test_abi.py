@@ -33,6 +33,8 @@ def test_library_exports_every_declared_symbol():
 def test_struct_layouts_match_header():
     assert ctypes.sizeof(B.TTParams) == 40
     assert B.HIT_DTYPE.itemsize == 16 and B.EVENT_DTYPE.itemsize == 32
+    assert B.RAW_DTYPE.itemsize == 16 and B.L1HIT_DTYPE.itemsize == 16  # tt_raw_hit, tt_l1hit: time first, like a hit
+    assert B.RAW_DTYPE.fields["t_ps"][1] == 0 and B.L1HIT_DTYPE.fields["t_ps"][1] == 0 and B.L1HIT_DTYPE.fields["idx"][1] == 8
     assert [B.TTParams.lc_window_ps.offset, B.TTParams.l2_window_ps.offset, B.TTParams.event_half_ps.offset,
             B.TTParams.l2_multiplicity.offset, B.TTParams.l2_mode.offset, B.TTParams.q_thresh.offset] == [0, 8, 16, 24, 28, 32]
 
@@ -50,6 +52,22 @@ def test_argument_errors_without_gpu():
     rc = lib.tt_sort_slice(z, z, z, ctypes.c_uint32(1000), z, bad.ctypes.data_as(ctypes.c_void_p), ctypes.c_uint32(1),
                            z, z, ctypes.c_uint32(0), z, ctypes.byref(need), z, z)
     assert rc == B.TT_E_INVAL
+    # workspace queries of the fused call and of the by-tower / preparation calls: host-only too
+    import ctypes as C
+
+    geo_dummy = (C.c_char * 64)()
+    prm = B.make_params()
+    rc = lib.tt_sort_trigger_slice(z, z, z, C.c_uint32(1000), z, seg.ctypes.data_as(C.c_void_p), C.c_uint32(1), z, z,
+                                   C.c_uint32(0), C.byref(geo_dummy), C.byref(prm), z, z, C.c_uint32(10), z, z, C.byref(need), z, z)
+    assert rc == 0 and need.value > 1000 * 60
+    rc = lib.tt_l1_export(z, C.c_uint32(1000), z, C.c_uint32(70000), z, C.c_uint32(0), z, z, C.byref(need), z, z)
+    assert rc == B.TT_E_INVAL  # src must fit 16 bits
+    rc = lib.tt_prepare_slice(z, z, C.c_uint32(1000), C.c_uint32(0), z, seg.ctypes.data_as(C.c_void_p), C.c_uint32(1),
+                              C.c_uint32(84), z, C.c_uint32(999), z, z, C.byref(need), z, z)
+    assert rc == B.TT_E_INVAL  # more raw hits than the output buffer holds
+    rc = lib.tt_prepare_slice(z, z, C.c_uint32(1000), C.c_uint32(0), z, seg.ctypes.data_as(C.c_void_p), C.c_uint32(1),
+                              C.c_uint32(84), z, C.c_uint32(1000), z, z, C.byref(need), z, z)
+    assert rc == 0 and need.value > 1000 * 24
     # runs that straddle a segment are rejected
     seg2 = np.array([0, 500, 1000], dtype=np.uint32)
     runs = np.array([0, 400, 1000], dtype=np.uint32)
