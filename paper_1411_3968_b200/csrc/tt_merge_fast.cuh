@@ -34,7 +34,7 @@ struct FastSmem {
 };
 static_assert(2 * (sizeof(FastSmem) + 1024) <= 233472, "two CTAs per SM");
 static_assert(offsetof(FastSmem, fl) % 16 == 0 && offsetof(FastSmem, cs) % 16 == 0 && offsetof(FastSmem, list) % 16 == 0, "16-byte accesses");
-static_assert(kFItems == 8, "the bucket scan reads two uint4 per thread");
+static_assert(kFItems == 8 && kFCap == 8 * kFThreads && kFCap < 65536, "the bucket scan: two uint4 per thread, two 16-bit partial sums in one word");
 
 __device__ __forceinline__ void bulk_s2g(void* dst, const void* src, uint32_t bytes) {
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(smem_u32(src)), "r"(bytes)
@@ -129,12 +129,6 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, L
     uint32_t fb[kFItems];    // composite high part (20 bits) << 12 | bucket
     uint32_t slot[kFItems];  // arrival position in the bucket, later start << 16 | count of the bucket
     bool unsorted = false;
-    if (check_runs && tid > 0 && tid < (uint32_t)kFCap / 32) {
-        // order across the 32-element groups of the loop below (its shuffle compares inside a group only): element
-        // 32 tid against its staged predecessor, unless it starts a piece
-        const uint32_t e = 32u * tid;
-        if (e < total && !(sm.pstart[tid] & 1u) && tile_key(sm.tile, e - 1) > tile_key(sm.tile, e)) unsorted = true;
-    }
 #pragma unroll
     for (int i = 0; i < kFItems; ++i) {
         const uint32_t e = tid + i * kFThreads;
@@ -146,10 +140,12 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, L
         const uint32_t hi = (v.y ^ 0x80000000u) - Ta_hi - (v.x < Ta_lo ? 1u : 0u);
         bool bad = hi != 0u || d >= width;
         if (check_runs) {
-            // order inside a run piece: the offset of the staged predecessor = the lane below
-            const uint32_t dp = __shfl_up_sync(0xffffffffu, d, 1);
+            // order inside a run piece: the offset of the staged predecessor = the lane below; lane 0 reads it (if the
+            // predecessor is outside [0, width) its own thread flags it, so comparing the low words is enough)
+            uint32_t dp = __shfl_up_sync(0xffffffffu, d, 1);
+            if (lane == 0u && e > 0u) dp = sm.tile[e - 1u].x - Ta_lo;
             const uint32_t ps = sm.pstart[(tid >> 5) + i * (kFThreads / 32)];  // one word per warp: a broadcast
-            bad |= lane != 0u && !((ps >> lane) & 1u) && dp > d;
+            bad |= e > 0u && !((ps >> lane) & 1u) && dp > d;
         }
         unsorted |= in_tile && bad;
         const uint64_t pr = (uint64_t)d * scale;
@@ -159,20 +155,24 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, L
         if (in_tile) slot[i] = atomicAdd(&sm.cs[b], 1u);
     }
     if (__syncthreads_or(unsorted) && tid == 0) atomicOr(status, TT_S_RUN_UNSORTED);
-    // ---- exclusive scan of the bucket counts: kFItems consecutive buckets per thread -> start << 16 | count
+    // ---- exclusive scan of the bucket counts -> start << 16 | count.  Every thread takes four consecutive buckets of
+    // the lower half and four of the upper half (two conflict-free 16-byte accesses; 8 consecutive buckets would be a
+    // 32-byte stride = two-way bank conflicts); both partial sums (<= kFCap each) ride in one 32-bit scan.
     {
         uint4* c4 = reinterpret_cast<uint4*>(sm.cs);
-        uint4 w0 = c4[2 * tid], w1 = c4[2 * tid + 1];
+        const uint4 w0 = c4[tid], w1 = c4[tid + kFThreads];
         uint32_t c[8] = {w0.x, w0.y, w0.z, w0.w, w1.x, w1.y, w1.z, w1.w};
-        uint32_t sum = 0;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) sum += c[i];
+        const uint32_t sum_lo = c[0] + c[1] + c[2] + c[3], sum_hi = c[4] + c[5] + c[6] + c[7];
         uint32_t tot;
-        uint32_t ex = block_scan1(sum, sm.scan + 16, &tot);
+        const uint32_t ex2 = block_scan1(sum_lo | (sum_hi << 16), sm.scan + 16, &tot);
+        uint32_t ex = ex2 & 0xFFFFu;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) { const uint32_t t = c[i]; c[i] = (ex << 16) | t; ex += t; }
-        c4[2 * tid] = make_uint4(c[0], c[1], c[2], c[3]);
-        c4[2 * tid + 1] = make_uint4(c[4], c[5], c[6], c[7]);
+        for (int i = 0; i < 4; ++i) { const uint32_t t = c[i]; c[i] = (ex << 16) | t; ex += t; }
+        ex = (tot & 0xFFFFu) + (ex2 >> 16);
+#pragma unroll
+        for (int i = 4; i < 8; ++i) { const uint32_t t = c[i]; c[i] = (ex << 16) | t; ex += t; }
+        c4[tid] = make_uint4(c[0], c[1], c[2], c[3]);
+        c4[tid + kFThreads] = make_uint4(c[4], c[5], c[6], c[7]);
     }
     __syncthreads();
     // ---- members of shared buckets go to the bucket's list
