@@ -2,6 +2,8 @@
 (one to several hundred per segment, two merge levels included), empty runs and segments, time distributions (uniform,
 clustered, heavy ties, wide spans), windows, multiplicities and modes drawn at random -- the shapes between the five
 configs and the hand-written edge cases."""
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -65,7 +67,12 @@ def _case(seed):
     return hits, np.asarray(seg, dtype=np.uint32), np.asarray(runs, dtype=np.uint32), single_tower_geo(tab), p
 
 
-@pytest.mark.parametrize("seed", range(36))
+# TT_FUZZ_FIRST / TT_FUZZ_SEEDS widen the sweep by hand (the default 36 seeds keep the suite short)
+_FIRST = int(os.environ.get("TT_FUZZ_FIRST", "0"))
+_COUNT = int(os.environ.get("TT_FUZZ_SEEDS", "36"))
+
+
+@pytest.mark.parametrize("seed", range(_FIRST, _FIRST + _COUNT))
 def test_random_chain(seed, B, oracle_lib):
     hits, seg, runs, g, p = _case(seed)
     o = oracle_chain(hits, seg, g, p)
