@@ -185,24 +185,33 @@ __global__ void __launch_bounds__(kFThreads, 2) merge_fast_kernel(LevelDev lv, L
         slot[i] = e < total ? w : 0u;
     }
     __syncthreads();
-    // ---- rank = bucket start + members of the bucket that order before this hit (four in a straight line: 99 % of
-    // the hits at a bucket load of 0.875; the loop is for the rare fuller buckets)
+    // ---- rank = bucket start + members of the bucket that order before this hit.  Four members in a straight line (99 %
+    // of the hits at a bucket load of 0.875), the loads of four hits issued together and predicated, no branch around
+    // them: a branch per hit serialised its four dependent shared-memory reads; the loop is for the rare fuller buckets
     uint32_t rk[kFItems];
 #pragma unroll
-    for (int i = 0; i < kFItems; ++i) {
-        const uint32_t e = tid + i * kFThreads;
-        const uint32_t s0 = slot[i] >> 16, cb = slot[i] & 0xFFFFu;
-        const uint32_t c = (fb[i] & 0xFFFFF000u) | e;
-        uint32_t r = s0;
-        if (cb > 1u) {
+    for (int h = 0; h < kFItems; h += 4) {
+        uint32_t o[4][4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t s0 = slot[h + u] >> 16, cb = slot[h + u] & 0xFFFFu;
             const uint32_t* const lp = sm.list + s0;
-            const uint32_t o0 = lp[0], o1 = lp[1];
-            const uint32_t o2 = cb > 2u ? lp[2] : 0xFFFFFFFFu, o3 = cb > 3u ? lp[3] : 0xFFFFFFFFu;
-            r += (o0 < c ? 1u : 0u) + (o1 < c ? 1u : 0u) + (o2 < c ? 1u : 0u) + (o3 < c ? 1u : 0u);
-#pragma unroll 1
-            for (uint32_t q = 4u; q < cb; ++q) r += lp[q] < c ? 1u : 0u;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) o[u][q] = (cb > 1u && cb > (uint32_t)q) ? lp[q] : 0xFFFFFFFFu;
         }
-        rk[i] = r;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const uint32_t e = tid + (h + u) * kFThreads;
+            const uint32_t s0 = slot[h + u] >> 16, cb = slot[h + u] & 0xFFFFu;
+            const uint32_t c = (fb[h + u] & 0xFFFFF000u) | e;
+            uint32_t r = s0 + (o[u][0] < c ? 1u : 0u) + (o[u][1] < c ? 1u : 0u) + (o[u][2] < c ? 1u : 0u) + (o[u][3] < c ? 1u : 0u);
+            if (cb > 4u) {
+                const uint32_t* const lp = sm.list + s0;
+#pragma unroll 1
+                for (uint32_t q = 4u; q < cb; ++q) r += lp[q] < c ? 1u : 0u;
+            }
+            rk[h + u] = r;
+        }
     }
     // ---- in-place permutation: all records to registers, one barrier, all records to their ranks
     uint4 rec[kFItems];
