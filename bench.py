@@ -269,6 +269,29 @@ def time_radix(B, run, peak):
             "note": "8-bit LSD passes over the varying key bits + one gather: ~5 passes x (12 B read + 24 B moved)"}
 
 
+def time_library_sort(B, run):
+    """Context, not a target and not on the product path: the library radix sort (torch.sort = CUB) of the int64 time keys of
+    this run's hits (keys + index; the 16-byte records would still have to be gathered through the index) next to this
+    repo's sort alone, tt_sort_slice with the permutation output, on the same device buffers."""
+    import torch
+
+    keys = run.d_in[:, 0].contiguous()
+    ms_lib = _cuda_time(lambda: torch.sort(keys, stable=True), 3)
+    del keys
+    st = torch.zeros(1, dtype=torch.int32, device="cuda")
+    perm = torch.empty(run.n, dtype=torch.int32, device="cuda")
+    ws = {}
+
+    def go():
+        ws["s"] = B.tt_sort_slice(run.d_in, run.d_out, perm, run.seg, run.runs, st, ws.get("s"))
+
+    ms_ours = _cuda_time(go, 3)
+    return {"workload": run.w.name, "hits": run.n, "library_sort_keys_and_index_ms": ms_lib,
+            "tt_sort_slice_records_and_perm_ms": ms_ours,
+            "note": "torch.sort(int64 keys, stable) ignores the per-PMT order of the input (PAPER.md:51-53 uses it) and "
+                    "moves 8-byte keys + 8-byte indices; tt_sort_slice moves the 16-byte records and a 4-byte permutation"}
+
+
 def time_streams(B, run, steps):
     """BASELINE.json configs[3]: "64 independent slices processed concurrently on one GPU through CUDA streams".  The
     same work as run.step(), but one call chain per segment (n_seg = 1) on its own stream, against the single
@@ -751,6 +774,11 @@ def run_ours(args):
             n_seeds_step = n_seeds
             extra["tower_shard"] = time_tower_shard(B, w, geo, prm, 8)
             assert extra["tower_shard"]["global_seeds"] == n_seeds_step, "by-tower path disagrees with the single-GPU path"
+        try:
+            extra["library_sort"] = time_library_sort(B, run)
+        except Exception as ex:  # context only: never takes the bench line down
+            extra["library_sort"] = {"error": type(ex).__name__}
+        torch.cuda.empty_cache()
         del run
         torch.cuda.empty_cache()
         for c2 in [c for c in (0, 1, 2, 3, 4) if c != args.config]:
