@@ -60,7 +60,10 @@ typedef struct {
     uint32_t l2_multiplicity; /* N >= 1, counts the hit itself; N <= TT_MAX_MULTIPLICITY           */
     uint32_t l2_mode;         /* 0 = clique ("N L1 hits pairwise causal"), 1 = star                */
     uint32_t q_thresh;        /* Q bit <=> charge >= q_thresh (0.01 p.e.; PAPER.md:64 QTRIG)       */
-    uint32_t reserved;        /* must be 0                                                         */
+    uint32_t l1_capacity;     /* 0: the L1 list may hold every hit (workspace ~69 B per hit).  Else the most L1
+                                 hits per call the trigger workspace is sized for (~69 B each; a detector has
+                                 2-8 % L1 hits): with more, TT_S_L1_OVERFLOW is set, the L1 flags of all hits
+                                 are still exact, and L2 / seeds see the first l1_capacity L1 hits in time order */
 } tt_params;
 
 /* One merged event window; 32 bytes.  Times are unclipped; [hit_begin, hit_end) indexes the sorted
@@ -81,7 +84,8 @@ enum {
     TT_S_EVENT_OVERFLOW = 2, /* likewise for events                                                   */
     TT_S_RUN_UNSORTED = 4,   /* a run given by d_run_offsets is not non-decreasing: output unspecified */
     TT_S_BAD_PMT = 8,        /* an L1 hit has pmt_id >= n_pmt (it has no L2 edges)                     */
-    TT_S_L1_OVERFLOW = 64,   /* tt_l1_export: more L1 hits than l1_cap (*d_n_l1 is the true count, first l1_cap valid)   */
+    TT_S_L1_OVERFLOW = 64,   /* tt_l1_export: more L1 hits than l1_cap (*d_n_l1 is the true count, first l1_cap valid);
+                                tt_trigger_slice / tt_sort_trigger_slice: more L1 hits than tt_params.l1_capacity      */
     TT_S_RAW_TRUNCATED = 32, /* tt_prepare_slice: a waveform reaches behind the sample section (missing samples = 0) */
     TT_S_DENSITY = 16        /* an L1 hit has more than TT_MAX_NEIGHBOURS L1 hits of its segment within
                                 +-min(W, largest table entry) of it: its L2STAR bit is exact, and its

@@ -38,7 +38,7 @@ class TTParams(ctypes.Structure):
     """Mirror of tt_params (40 bytes)."""
     _fields_ = [("lc_window_ps", ctypes.c_int64), ("l2_window_ps", ctypes.c_int64),
                 ("event_half_ps", ctypes.c_int64), ("l2_multiplicity", c_u32), ("l2_mode", c_u32),
-                ("q_thresh", c_u32), ("reserved", c_u32)]
+                ("q_thresh", c_u32), ("l1_capacity", c_u32)]
 
 
 assert ctypes.sizeof(TTParams) == 40
@@ -115,9 +115,9 @@ def _stream() -> c_vp:
 
 
 def make_params(q_thresh=300, lc_window_ps=20_000, l2_window_ps=3_000_000, l2_multiplicity=5, l2_mode=0,
-                event_half_ps=3_000_000) -> TTParams:
+                event_half_ps=3_000_000, l1_capacity=0) -> TTParams:
     return TTParams(int(lc_window_ps), int(l2_window_ps), int(event_half_ps), int(l2_multiplicity), int(l2_mode),
-                    int(q_thresh), 0)
+                    int(q_thresh), int(l1_capacity))
 
 
 class Geometry:

@@ -305,7 +305,7 @@ extern "C" int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint3
                                  tt_hit* d_gather, uint32_t* d_n_gathered, void* d_ws, size_t* ws_bytes,
                                  int32_t* d_status, void* stream) {
     if (!ws_bytes || !p || n_seg < 1 || !h_seg_offsets) return TT_E_INVAL;
-    if (p->event_half_ps < 0 || p->reserved != 0) return TT_E_INVAL;
+    if (p->event_half_ps < 0) return TT_E_INVAL;
     if (n >= 0xFFF00000u) return TT_E_INVAL;
     if (h_seg_offsets[0] != 0 || h_seg_offsets[n_seg] != n) return TT_E_INVAL;
     Arena sizing(nullptr);

@@ -323,9 +323,16 @@ __global__ void __launch_bounds__(kL1Threads) l1_count_kernel(const uint8_t* __r
 __global__ void __launch_bounds__(kL1Threads) l1_compact_kernel(const uint4* __restrict__ hits, uint32_t n,
                                                                 const uint8_t* __restrict__ flags,
                                                                 const uint32_t* __restrict__ tile_off,
-                                                                L1Rec* __restrict__ l1, uint32_t n_pmt, uint32_t ppt,
-                                                                int32_t* __restrict__ status) {
+                                                                L1Rec* __restrict__ l1, uint32_t cap,
+                                                                uint32_t* __restrict__ m_total, uint32_t n_pmt,
+                                                                uint32_t ppt, int32_t* __restrict__ status) {
     __shared__ uint32_t sm[33];
+    // the list holds cap records (tt_params.l1_capacity): later L1 hits keep their flags but are not listed.  No block of
+    // this kernel reads *m_total; the L2 kernels that follow see the clamped count.
+    if (blockIdx.x == 0 && threadIdx.x == 0 && *m_total > cap) {
+        *m_total = cap;
+        atomicOr(status, TT_S_L1_OVERFLOW);
+    }
     const uint32_t i0 = blockIdx.x * (uint32_t)kL1Tile + threadIdx.x * kL1Per;
     uint32_t mask = 0;
     if (i0 < n) {
@@ -364,7 +371,7 @@ __global__ void __launch_bounds__(kL1Threads) l1_compact_kernel(const uint4* __r
         rec.idx = i;
         if (h.pmt >= n_pmt) { rec.tp = kBadTp; bad = true; }
         else { const uint32_t tw = h.pmt / ppt; rec.tp = (tw << 16) | (h.pmt - tw * ppt); }
-        l1[base + q] = rec;
+        if (base + q < cap) l1[base + q] = rec;
     }
     if (__syncthreads_or(bad) && threadIdx.x == 0) atomicOr(status, TT_S_BAD_PMT);
 }
@@ -1059,16 +1066,19 @@ struct TriggerPlan {
     uint32_t nblk;
 };
 
-static void trigger_plan(Arena& a, uint32_t n, TriggerPlan& p) {
+// cap: L1 hits the list arrays hold (n, or tt_params.l1_capacity if that is smaller)
+static uint32_t l1_cap(uint32_t n, const tt_params* p) { return p->l1_capacity && p->l1_capacity < n ? p->l1_capacity : n; }
+
+static void trigger_plan(Arena& a, uint32_t n, uint32_t cap, TriggerPlan& p) {
     p.nblk = div_up(n, kL1Tile);
     p.blk_cnt = a.take<uint32_t>(p.nblk + 1);
     p.scan_scratch = a.take<uint32_t>(scan_ws_count(p.nblk + 1));
     p.m_total = a.take<uint32_t>(1);
     p.seed_cnt = a.take<uint32_t>(kSeedBlocks);
-    p.l1 = a.take<L1Rec>(n);
-    p.l2bit = a.take<uint8_t>(n);
-    p.rows = a.take<Row>(n);
-    p.slow_list = a.take<uint32_t>(n);
+    p.l1 = a.take<L1Rec>(cap);
+    p.l2bit = a.take<uint8_t>(cap);
+    p.rows = a.take<Row>(cap);
+    p.slow_list = a.take<uint32_t>(cap);
     p.slow_cnt = a.take<uint32_t>(4);  // [0] slow-list length, [1] / [2] tile counters of the rows / clique kernels
 }
 
@@ -1088,7 +1098,7 @@ static int trigger_attrs() {
 static int trigger_args_ok(uint32_t n, const uint32_t* h_seg_offsets, uint32_t n_seg, const tt_geometry* g,
                            const tt_params* p) {
     if (!p || !g || n_seg < 1 || !h_seg_offsets) return TT_E_INVAL;
-    if (p->l2_multiplicity < 1 || p->l2_multiplicity > TT_MAX_MULTIPLICITY || p->l2_mode > 1 || p->reserved != 0 ||
+    if (p->l2_multiplicity < 1 || p->l2_multiplicity > TT_MAX_MULTIPLICITY || p->l2_mode > 1 ||
         p->lc_window_ps < 0 || p->l2_window_ps < 0 || p->event_half_ps < 0)
         return TT_E_INVAL;
     if (n >= 0xFFF00000u) return TT_E_INVAL;
@@ -1109,7 +1119,8 @@ static int trigger_run(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg
                        uint32_t* d_n_seeds, void* d_ws, int32_t* d_status, cudaStream_t s, const MergeLast* last) {
     Arena a(d_ws);
     TriggerPlan plan;
-    trigger_plan(a, n, plan);
+    const uint32_t cap = l1_cap(n, p);
+    trigger_plan(a, n, cap, plan);
     int rc = once_per_device(kSlotTrigger, trigger_attrs);
     if (rc != TT_OK) return rc;
     const uint32_t sms = (uint32_t)sm_count();
@@ -1129,7 +1140,7 @@ static int trigger_run(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg
     if (rc != TT_OK) return rc;
     prof_mark(s, "trig.l1_compact");
     TT_K(l1_compact_kernel)<<<plan.nblk, kL1Threads, 0, s>>>((const uint4*)d_sorted, n, d_flags, plan.blk_cnt, plan.l1,
-                                                         g->dev.n_pmt, g->dev.ppt, d_status);
+                                                         cap, plan.m_total, g->dev.n_pmt, g->dev.ppt, d_status);
     return trigger_l2(plan, n, d_seg_offsets, n_seg, g, p, d_flags, d_seeds, seed_cap, d_n_seeds, d_status, s);
 }
 
@@ -1175,7 +1186,7 @@ extern "C" int tt_trigger_slice(const tt_hit* d_sorted, uint32_t n, const uint32
     if (rc != TT_OK) return rc;
     Arena sizing(nullptr);
     TriggerPlan plan;
-    trigger_plan(sizing, n, plan);
+    trigger_plan(sizing, n, l1_cap(n, p), plan);
     if (!d_ws) {
         *ws_bytes = sizing.off;
         return TT_OK;
@@ -1476,7 +1487,7 @@ extern "C" int tt_l2_merged(const tt_l1hit* d_l1, uint32_t m, const tt_geometry*
     if (rc != TT_OK) return rc;
     Arena sizing(nullptr);
     TriggerPlan plan;
-    trigger_plan(sizing, m, plan);
+    trigger_plan(sizing, m, m, plan);
     if (!d_ws) {
         *ws_bytes = sizing.off;
         return TT_OK;
@@ -1489,7 +1500,7 @@ extern "C" int tt_l2_merged(const tt_l1hit* d_l1, uint32_t m, const tt_geometry*
         return TT_OK;
     }
     Arena a(d_ws);
-    trigger_plan(a, m, plan);
+    trigger_plan(a, m, m, plan);
     rc = once_per_device(kSlotTrigger, trigger_attrs);
     if (rc != TT_OK) return rc;
     prof_mark(s, "towers.l2_prepare");

@@ -192,6 +192,56 @@ def test_fused_status_and_capacity(B, oracle_lib):
     assert (r.status & B.TT_S_BAD_PMT) and (r.flags == o2["flags"]).all()
 
 
+@pytest.mark.parametrize("fused", [True, False])
+@pytest.mark.parametrize("cfg,ts", [(2, 0.004), (4, 0.004)])
+def test_l1_capacity(cfg, ts, fused, B, oracle_lib):
+    """tt_params.l1_capacity bounds the L1 list (and with it the trigger workspace).  Enough room: the oracle's bytes.
+    Too little: TT_S_L1_OVERFLOW, every L1 flag still exact, L2 over the first l1_capacity L1 hits in time order -- so no
+    L2 bit the full answer does not have, and the full answer wherever the window of a hit ends before the cut."""
+    w = W.make_config(cfg, time_scale=ts)
+    g, p = w.geometry, w.params
+    o = oracle_chain(w.hits, w.seg_offsets, g, p)
+    m = int(((o["flags"] & B.TT_L1) != 0).sum())
+    assert m > 200
+    geo = _geo(B, g)
+
+    def prm(cap):
+        return B.make_params(p.q_thresh, p.lc_window_ps, p.l2_window_ps, p.l2_multiplicity, p.l2_mode, p.event_half_ps,
+                             l1_capacity=cap)
+
+    for cap in (m, m + 17, len(w.hits) + 5):  # room for every L1 hit
+        r = B.process_slice(w.hits, w.seg_offsets, w.run_offsets, geo, prm(cap), fused=fused)
+        assert r.status == 0, cap
+        _compare(r, o)
+    cap = m // 2
+    r = B.process_slice(w.hits, w.seg_offsets, w.run_offsets, geo, prm(cap), fused=fused)
+    assert r.status & B.TT_S_L1_OVERFLOW
+    assert r.sorted.tobytes() == o["sorted"].tobytes()
+    assert ((r.flags & 7) == (o["flags"] & 7)).all()                    # Q, LC, L1: all hits
+    l2 = B.TT_L2 | B.TT_L2STAR
+    assert ((r.flags & l2) & ~(o["flags"] & l2) == 0).all()             # fewer L1 hits listed: never more L2 bits
+    l1_pos = np.nonzero(o["flags"] & B.TT_L1)[0]
+    t_cut = int(o["sorted"]["t_ps"][l1_pos[cap]])                        # first L1 hit that is not listed
+    reach = min(int(p.l2_window_ps), int(g.blocks.max()))
+    early = o["sorted"]["t_ps"] < t_cut - reach                          # windows that end before the cut (one segment)
+    assert early.sum() > 0 and ((r.flags & l2)[early] == (o["flags"] & l2)[early]).all()
+    assert (r.flags[l1_pos[cap:]] & l2 == 0).all()                       # unlisted L1 hits: no L2 bit
+    # the workspace follows the capacity
+    n = len(w.hits)
+    import ctypes
+    need = {}
+    for c in (0, cap):
+        nb = ctypes.c_size_t(0)
+        pr = prm(c)
+        rc = B.load().tt_trigger_slice(None, ctypes.c_uint32(n), None, w.seg_offsets.ctypes.data_as(ctypes.c_void_p),
+                                       ctypes.c_uint32(len(w.seg_offsets) - 1), geo.handle, ctypes.byref(pr), None, None,
+                                       ctypes.c_uint32(n), None, None, ctypes.byref(nb), None, None)
+        assert rc == 0
+        need[c] = nb.value
+    assert need[cap] < need[0] and need[0] - need[cap] >= 60 * (n - cap)
+    geo.close()
+
+
 @pytest.mark.parametrize("cfg,ts,ss", [(2, 0.01, 1), (3, 0.02, 8 / 64), (4, 0.004, 1)])
 def test_fused_graph_replay_dirty_buffers(cfg, ts, ss, B, oracle_lib):
     """bench.py's step with the fused call: captured in a CUDA graph, replayed onto garbage-filled outputs and
