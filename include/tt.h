@@ -63,7 +63,7 @@ typedef struct {
     uint32_t l1_capacity;     /* 0: the L1 list may hold every hit (workspace ~69 B per hit).  Else the most L1
                                  hits per call the trigger workspace is sized for (~69 B each; a detector has
                                  2-8 % L1 hits): with more, TT_S_L1_OVERFLOW is set, the L1 flags of all hits
-                                 are still exact, and L2 / seeds see the first l1_capacity L1 hits in time order */
+                                 are still exact, and L2 / seeds see the first l1_capacity L1 hits of the sorted array  */
 } tt_params;
 
 /* One merged event window; 32 bytes.  Times are unclipped; [hit_begin, hit_end) indexes the sorted
