@@ -76,7 +76,8 @@ typedef struct {
 /* per-hit flag byte */
 enum { TT_Q = 1, TT_LC = 2, TT_L1 = 4, TT_L2STAR = 8, TT_L2 = 16, TT_INEVT = 32 };
 /* return codes */
-enum { TT_OK = 0, TT_E_INVAL = -1, TT_E_CUDA = -2, TT_E_WORKSPACE = -3 };
+enum { TT_OK = 0, TT_E_INVAL = -1, TT_E_CUDA = -2, TT_E_WORKSPACE = -3,
+       TT_E_LIMIT = -4 /* tt_extract_events_noalloc: the request needs more than TT_NOALLOC_WS_BYTES of scratch */ };
 /* *d_status bits */
 enum {
     TT_S_OK = 0,
@@ -159,6 +160,26 @@ int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_
                       tt_event* d_events, uint32_t event_cap, uint32_t* d_n_events, uint8_t* d_flags,
                       tt_hit* d_gather, uint32_t* d_n_gathered, void* d_ws, size_t* ws_bytes,
                       int32_t* d_status, void* stream);
+
+/* tt_extract_events for callers that cannot allocate device memory (code under CUDA-graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same operation, the same arguments minus the
+ * workspace pair, the same outputs byte for byte -- the scratch the kernels need (per-block counts, the head flag of
+ * every seed, the gather offset of every event: 4 * event_cap + seed_cap + ~5 KB) lives in a static device array of
+ * TT_NOALLOC_WS_BYTES inside the library, which every GPU that loads the library holds until the process exits.
+ *   - seed_cap / event_cap whose scratch does not fit return TT_E_LIMIT and launch nothing (e.g. event_cap = 2^18
+ *     with seed_cap = 2^21 fits; cfg4 has 1.18 M seeds and 405 events per slice);
+ *   - the call makes no cudaMalloc / cudaFree and calls no allocating library routine; the first call on a device
+ *     resolves the array's device address (cudaGetSymbolAddress, once per device, that device current), so make that
+ *     first call outside stream capture;
+ *   - ALL calls on a device share the one array, which keeps the last call's contents (nothing in it has to start at
+ *     zero: every word a kernel reads was written earlier in the same call): two calls that overlap on the GPU
+ *     (different streams, no dependency between them) race on it.  Calls on one stream are ordered and safe. */
+#define TT_NOALLOC_WS_BYTES (4u << 20)
+int tt_extract_events_noalloc(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets,
+                              const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* d_seeds,
+                              const uint32_t* d_n_seeds, uint32_t seed_cap, const tt_params* p,
+                              tt_event* d_events, uint32_t event_cap, uint32_t* d_n_events, uint8_t* d_flags,
+                              tt_hit* d_gather, uint32_t* d_n_gathered, int32_t* d_status, void* stream);
 
 /* Level-0 N-in-TW trigger on time-sorted hits: "N7TW1000: looking for 7 hits
  * in TW = 1000 ns: hit[i].time-hit[i+7].time< TW", PAPER.md:73 (N7TW500 for the 84-PMT tower), PAPER.md:67 (applied

@@ -19,6 +19,8 @@ c_u32, c_i32, c_vp, c_sz = ctypes.c_uint32, ctypes.c_int32, ctypes.c_void_p, cty
 
 TT_Q, TT_LC, TT_L1, TT_L2STAR, TT_L2, TT_INEVT = 1, 2, 4, 8, 16, 32
 TT_OK, TT_E_INVAL, TT_E_CUDA, TT_E_WORKSPACE = 0, -1, -2, -3
+TT_E_LIMIT = -4
+TT_NOALLOC_WS_BYTES = 4 << 20
 TT_S_SEED_OVERFLOW, TT_S_EVENT_OVERFLOW, TT_S_RUN_UNSORTED, TT_S_BAD_PMT, TT_S_DENSITY = 1, 2, 4, 8, 16
 TT_S_RAW_TRUNCATED = 32
 TT_S_L1_OVERFLOW = 64
@@ -27,7 +29,8 @@ EXPORTS = ["tt_version", "tt_geometry_create", "tt_geometry_destroy", "tt_sort_s
            "tt_extract_events", "tt_host_ctx_create", "tt_host_ctx_destroy", "tt_process_host", "tt_launch_count",
            "tt_prof_enable", "tt_prof_read", "tt_l0_ntw", "tt_pair_seeds", "tt_l0_combine",
            "tt_l0_dntw", "tt_sort_trigger_slice", "tt_prepare_slice", "tt_host_submit",
-           "tt_host_wait", "tt_sort_l1_slice", "tt_l1_export", "tt_l2_merged", "tt_l2_apply", "tt_tag_windows"]
+           "tt_host_wait", "tt_sort_l1_slice", "tt_l1_export", "tt_l2_merged", "tt_l2_apply", "tt_tag_windows",
+           "tt_extract_events_noalloc"]
 
 HIT_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("charge", "<u2"), ("pad", "<u2")])
 EVENT_DTYPE = np.dtype([("t_start", "<i8"), ("t_end", "<i8"), ("hit_begin", "<u4"), ("hit_end", "<u4"),
@@ -264,6 +267,24 @@ def tt_extract_events(d_sorted: torch.Tensor, seg: Offsets, d_seeds: torch.Tenso
     nb = c_sz(ws.numel())
     _check(call(_dp(ws), ctypes.byref(nb)), "tt_extract_events")
     return ws
+
+
+def tt_extract_events_noalloc(d_sorted: torch.Tensor, seg: Offsets, d_seeds: torch.Tensor, d_n_seeds: torch.Tensor,
+                              params: TTParams, d_events: torch.Tensor, d_n_events: torch.Tensor,
+                              d_flags: torch.Tensor | None, d_gather: torch.Tensor | None,
+                              d_n_gathered: torch.Tensor | None, d_status: torch.Tensor) -> int:
+    """tt_extract_events with the scratch in the library's static device array: no workspace, nothing allocated.
+    Returns the call's code (TT_OK or TT_E_LIMIT when seed_cap / event_cap need more than TT_NOALLOC_WS_BYTES);
+    raises on any other error."""
+    _need_cuda()
+    L = load()
+    rc = L.tt_extract_events_noalloc(_dp(d_sorted), c_u32(d_sorted.shape[0]), _dp(seg.d), _hp(seg.h), c_u32(seg.count),
+                                     _dp(d_seeds), _dp(d_n_seeds), c_u32(d_seeds.numel()), ctypes.byref(params),
+                                     _dp(d_events), c_u32(d_events.shape[0]), _dp(d_n_events), _dp(d_flags),
+                                     _dp(d_gather), _dp(d_n_gathered), _dp(d_status), _stream())
+    if rc != TT_E_LIMIT:
+        _check(rc, "tt_extract_events_noalloc")
+    return rc
 
 
 RAW_DTYPE = np.dtype([("t_ps", "<i8"), ("pmt_id", "<u2"), ("floor", "<u2"), ("n_samples", "<u2"), ("pad", "<u2")])

@@ -5,6 +5,8 @@
 //   never across a segment; t_start / t_end unclipped.
 #include "tt_common.cuh"
 
+#include <mutex>
+
 namespace tt {
 
 constexpr int kEvBlocks = 592;  // fixed grid: the seed count lives on the device
@@ -353,4 +355,47 @@ extern "C" int tt_extract_events(const tt_hit* d_sorted, uint32_t n, const uint3
     prof_end(s);
     TT_LAUNCH_OK();
     return TT_OK;
+}
+
+// ---- the same call with its scratch in a static device array (tt.h: tt_extract_events_noalloc) -------------------
+// In host code `g_noalloc_ws` is a host-side stand-in for the symbol, not a device address: the address the kernels
+// get comes from cudaGetSymbolAddress, looked up once per device with that device current.
+static __device__ __align__(256) unsigned char g_noalloc_ws[TT_NOALLOC_WS_BYTES];
+
+static int noalloc_ws_address(void** out) {
+    constexpr int kMaxDev = 64;
+    static std::mutex mu;
+    static void* addr[kMaxDev];  // zero-initialised
+    int dev = -1;
+    TT_CUDA_OK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDev) return TT_E_CUDA;
+    std::lock_guard<std::mutex> lk(mu);
+    if (!addr[dev]) {
+        void* p = nullptr;
+        TT_CUDA_OK(cudaGetSymbolAddress(&p, g_noalloc_ws));
+        if (!p || ((uintptr_t)p & 255)) return TT_E_CUDA;
+        addr[dev] = p;
+    }
+    *out = addr[dev];
+    return TT_OK;
+}
+
+extern "C" int tt_extract_events_noalloc(const tt_hit* d_sorted, uint32_t n, const uint32_t* d_seg_offsets,
+                                         const uint32_t* h_seg_offsets, uint32_t n_seg, const uint32_t* d_seeds,
+                                         const uint32_t* d_n_seeds, uint32_t seed_cap, const tt_params* p,
+                                         tt_event* d_events, uint32_t event_cap, uint32_t* d_n_events,
+                                         uint8_t* d_flags, tt_hit* d_gather, uint32_t* d_n_gathered,
+                                         int32_t* d_status, void* stream) {
+    // argument errors first (the size query of the general call checks them), then the limit
+    size_t need = 0;
+    int rc = tt_extract_events(d_sorted, n, d_seg_offsets, h_seg_offsets, n_seg, d_seeds, d_n_seeds, seed_cap, p, d_events,
+                               event_cap, d_n_events, d_flags, d_gather, d_n_gathered, nullptr, &need, d_status, stream);
+    if (rc != TT_OK) return rc;
+    if (need > (size_t)TT_NOALLOC_WS_BYTES) return TT_E_LIMIT;
+    void* ws = nullptr;
+    rc = noalloc_ws_address(&ws);
+    if (rc != TT_OK) return rc;
+    size_t have = TT_NOALLOC_WS_BYTES;
+    return tt_extract_events(d_sorted, n, d_seg_offsets, h_seg_offsets, n_seg, d_seeds, d_n_seeds, seed_cap, p, d_events,
+                             event_cap, d_n_events, d_flags, d_gather, d_n_gathered, ws, &have, d_status, stream);
 }
